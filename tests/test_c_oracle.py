@@ -1,0 +1,99 @@
+"""The plain-C oracle (oracle/pn_oracle.c) against the same pins as the Python one, and against it."""
+import numpy as np
+import pytest
+
+from oracle import c_oracle, pn_oracle as po
+from paper_1908_03301_b200 import inputs
+from test_oracle_pins import brute_force_dense, independent_classes
+
+
+def crun(net, direction=0, tol=1e-13, **kw):
+    return c_oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, tol, **kw)
+
+
+@pytest.mark.parametrize("shape,direction", [((9, 6, 5), 0), ((9, 6, 5), 1), ((9, 6, 5), 2), ((7, 4, 1), 1)])
+def test_c_oracle_uniform(shape, direction):
+    nx, ny, nz = shape
+    res = crun(inputs.uniform(nx, ny, nz, 0.37), direction)
+    n_a = shape[direction]
+    coord = po._coord_along(nx, ny, nz, direction)[0]
+    assert np.max(np.abs(res.P - (1.0 - coord / (n_a - 1)))) < 1e-12
+    g32 = float(np.float32(0.37))
+    assert res.g_eff == pytest.approx(g32 * (nx * ny * nz // n_a) / (n_a - 1), rel=1e-12)
+    assert res.k_eff == pytest.approx(g32, rel=1e-12)
+
+
+def test_c_oracle_layered_means():
+    nx, ny, nz = 6, 5, 7
+    rng = np.random.default_rng(11)
+    c = rng.uniform(0.2, 3.0, nz).astype(np.float32)
+    e = rng.uniform(0.2, 3.0, nz).astype(np.float32)
+    net = inputs.layered_exact(nx, ny, nz, c, e)
+    assert crun(net, 0).g_eff == pytest.approx(ny * c.astype(float).sum() / (nx - 1), rel=1e-12)
+    assert crun(net, 2).g_eff == pytest.approx(nx * ny / np.sum(1.0 / e.astype(float)[:nz - 1]), rel=1e-12)
+
+
+def test_c_oracle_worked_example():
+    gx = np.zeros((1, 2, 3), np.float32)
+    gy = np.zeros((1, 2, 3), np.float32)
+    gx[0, 0, 0], gx[0, 0, 1], gx[0, 1, 0], gx[0, 1, 1] = 1, 2, 3, 4
+    gy[0, 0, 1] = 5
+    gx[0, :, 2] = 99.0
+    gy[0, 1, :] = 77.0
+    res = crun(inputs.Network(3, 2, 1, gx, gy, None), 0)
+    assert res.P[0, 0, 1] == pytest.approx(27 / 71, rel=1e-13)
+    assert res.P[0, 1, 1] == pytest.approx(29 / 71, rel=1e-13)
+    assert res.q_in == pytest.approx(170 / 71, rel=1e-13)
+    assert res.q_out == pytest.approx(170 / 71, rel=1e-13)
+
+
+@pytest.mark.parametrize("shape,p,seed,direction", [
+    ((6, 5, 1), 0.7, 2, 1), ((5, 4, 3), 0.6, 4, 0), ((4, 5, 4), 0.5, 5, 1), ((16, 16, 1), 0.65, 7, 0),
+    ((7, 6, 5), 0.45, 8, 2)])
+def test_c_oracle_dense_bruteforce_and_labels(shape, p, seed, direction):
+    net = inputs.iid_diluted(*shape, seed=seed, p=p)
+    res = crun(net, direction)
+    Pd, _ = brute_force_dense(net, direction)
+    defined = res.classes != po.FLOATING
+    assert np.max(np.abs(res.P[defined] - Pd[defined])) < 1e-11
+    assert np.array_equal(res.classes, independent_classes(net, direction))
+
+
+@pytest.mark.parametrize("maker,direction", [
+    (lambda: inputs.cfg1_iid_2d(64, 64, seed=0), 0),
+    (lambda: inputs.cfg2_fbm_2d(48, 40, seed=1), 0),
+    (lambda: inputs.cfg3_percolation_3d(20, 18, 16, seed=2, p=0.35), 0),
+    (lambda: inputs.cfg4_fbm_cut_3d(20, 20, 20, seed=3), 1),
+    (lambda: inputs.cfg5_stratified_3d(16, 14, 18, seed=4), 2),
+])
+def test_c_oracle_matches_python_oracle(maker, direction):
+    net = maker()
+    a = po.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13)
+    b = crun(net, direction)
+    assert np.array_equal(a.classes, b.classes)
+    assert (a.n_solved, a.n_inlet_only, a.n_outlet_only, a.n_floating) == \
+           (b.n_solved, b.n_inlet_only, b.n_outlet_only, b.n_floating)
+    assert np.max(np.abs(a.P - b.P)) < 1e-11
+    assert b.g_eff == pytest.approx(a.g_eff, rel=1e-11)
+    assert b.q_in == pytest.approx(a.q_in, rel=1e-11) and b.q_out == pytest.approx(a.q_out, rel=1e-11)
+    assert b.rel_residual <= 1e-13 and b.status == "ok"
+    rel, pin = c_oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, a.P, direction)
+    assert rel <= 1e-13 and pin == 0.0
+    relp, _ = po.residual_certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, b.P, direction)
+    assert relp <= 1e-13
+
+
+def test_c_oracle_no_spanning_cluster_and_errors():
+    net = inputs.iid_diluted(30, 30, 1, seed=3, p=0.2)
+    res = crun(net, 0)
+    assert res.status == "no_spanning_cluster" and res.g_eff == 0.0
+    bad = inputs.uniform(4, 4, 1, 1.0)
+    bad.gx[0, 1, 1] = -2.0
+    with pytest.raises(ValueError):
+        crun(bad, 0)
+    with pytest.raises(ValueError):
+        crun(inputs.uniform(2, 4, 1, 1.0), 0)
+    # max_iter is honoured and reported
+    net = inputs.cfg1_iid_2d(32, 32, seed=0)
+    r = crun(net, 0, tol=1e-13, max_iter=5)
+    assert r.status == "max_iters" and r.iterations == 5 and r.rel_residual > 1e-13
