@@ -1,0 +1,144 @@
+/* pn.h -- C ABI of libpn: mixed-precision conjugate-gradient solve of bond-network Kirchhoff systems
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * The problem (citations: /root/reference/PAPER.md = P:<line>; SURVEY.md section 8 = S8):
+ *   nodes of a square (nz == 1) or simple-cubic lattice nx x ny x nz, node n = i + nx*(j + ny*k);
+ *   bonds with conductance g_ij >= 0 (g == 0: closed bond); flow in a bond q_ij = g_ij (P_j - P_i)
+ *   mass balance at every interior node  sum_j g_ij (P_i - P_j) = 0  ->  G P = b, eq.(3)
+ *   a fixed macroscopic pressure drop along one lattice axis `a`: P = 1 on the node plane coord_a = 0,
+ *   P = 0 on the plane coord_a = n_a - 1; every other face is a no-flux face                        P:57, S8(c) 1-2
+ *   (the paper's lateral faces are periodic; BASELINE.json's north_star and configs[0] fix no-flux)
+ *   solved by conjugate gradients, single precision inside, double precision outside
+ *   then total flow Q through a cross-section and Darcy permeability K = (Q/S)(mu L/dP), eq.(4)
+ *
+ * Conductance arrays (S8(a)): three (two in 2D) float arrays of nx*ny*nz entries each, x fastest,
+ * FORWARD-BOND convention:  gx[n] = bond (i,j,k)--(i+1,j,k),  gy[n] = bond (i,j,k)--(i,j+1,k),
+ * gz[n] = bond (i,j,k)--(i,j,k+1).  Entries whose forward neighbour is outside the lattice are not
+ * bonds; they are ignored whatever they hold.  The float values ARE the problem: the double
+ * precision steps widen exactly these values (S8(c) reading 14).
+ *
+ * Ownership: the caller owns every device buffer (workspace, inputs, outputs).  The library owns
+ * the host-side handle and a few hundred bytes of pinned host memory.  All device work is enqueued
+ * on the stream given to pn_create.  A handle is not thread-safe; distinct handles are independent.
+ * No call prints, aborts or throws.  There is no CPU fallback: without a CUDA device every call
+ * that needs one returns PN_ERR_CUDA.
+ */
+#ifndef PN_H
+#define PN_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pn_ctx pn_ctx; /* opaque handle: one network on one device / stream */
+
+/* return codes: 0 ok, > 0 valid non-error outcomes, < 0 errors */
+enum {
+    PN_OK = 0,
+    PN_NO_SPANNING_CLUSTER = 1, /* no cluster joins inlet and outlet: Q = 0, pressures = pin values */
+    PN_MAX_ITERS = 2,           /* iteration budget spent or residual stagnated; best iterate kept  */
+    PN_ERR_ARG = -1,            /* null pointer, bad shape / direction / tol, axis shorter than 3   */
+    PN_ERR_STATE = -2,          /* solve before set_conductances, flux / pressures before solve     */
+    PN_ERR_VALUE = -3,          /* negative, NaN or Inf conductance on an in-lattice bond           */
+    PN_ERR_WORKSPACE = -4,      /* workspace missing, misaligned (256 B) or too small               */
+    PN_ERR_CUDA = -5,           /* a CUDA call failed (sticky; pn_last_error has the text)          */
+    PN_ERR_BREAKDOWN = -6       /* CG breakdown: p.Ap <= 0 or non-finite                            */
+};
+
+/* node classes written by pn_get_classes (S8(c) steps 2-3) */
+enum {
+    PN_CLASS_INLET = 0,       /* Dirichlet plane coord_a = 0,        P = 1                          */
+    PN_CLASS_OUTLET = 1,      /* Dirichlet plane coord_a = n_a - 1,  P = 0                          */
+    PN_CLASS_SOLVED = 2,      /* interior node of a cluster that reaches both planes: unknown       */
+    PN_CLASS_INLET_ONLY = 3,  /* cluster reaches only the inlet:  no flow, P = 1 exactly (pinned)   */
+    PN_CLASS_OUTLET_ONLY = 4, /* cluster reaches only the outlet: no flow, P = 0 exactly (pinned)   */
+    PN_CLASS_FLOATING = 5     /* cluster reaches neither: P undefined, pinned to 0 by convention    */
+};
+
+typedef struct {
+    int status;            /* the code pn_solve returned                                            */
+    int outer_cycles;      /* fp64 true-residual evaluations  r = b - A x  (S8(a) S3)                */
+    int inner_iters;       /* fp32 CG iterations (S8(a) S4+S5), summed over the solve               */
+    int reserved;
+    double rel_residual;   /* true fp64 ||b - A x||_2 / ||b||_2 over the solved nodes at exit       */
+    double b_norm;         /* ||b||_2 of the zero-initial-guess system (S8(c) reading 5)            */
+    long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
+    double t_label_ms;     /* S1 + set-up (labelling, pruning, scaling), device time                */
+    double t_solve_ms;     /* S3..S7 loop, device time                                              */
+} pn_info;
+
+/* options for pn_set_option */
+enum {
+    PN_OPT_MAX_ITERS = 0,   /* inner-iteration budget per solve            (default 200000)         */
+    PN_OPT_DELTA = 1,       /* reliable-update threshold: fp64 residual replacement when the fp32
+                               recursive residual has fallen by this factor since the last one
+                               (default 0.1; S8(c) reading 4)                                       */
+    PN_OPT_X0 = 2,          /* initial guess on solved nodes: 0 = zero, 1 = linear profile along the
+                               solve axis (default 1; S8(c) reading 6)                              */
+    PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32)            */
+    PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
+                               S1 is always skipped automatically when no in-lattice g == 0 exists) */
+    PN_OPT_KERNEL = 5       /* S4 kernel variant: 0 = default (fastest), 1 = reference kernel that
+                               reads neighbours through the caches (kept for cross-checks)          */
+};
+
+/* Device bytes pn_create needs for an nx x ny x nz lattice (0 on a bad shape). */
+size_t pn_workspace_bytes(int nx, int ny, int nz);
+
+/* Create a handle.  nx, ny, nz >= 1 (nz == 1: 2D).  `device`: CUDA ordinal.  `cuda_stream`: a
+ * cudaStream_t (NULL = the legacy default stream).  `workspace`: DEVICE memory, 256-byte aligned, at
+ * least pn_workspace_bytes(nx, ny, nz) bytes, owned by the caller and left untouched by it until
+ * pn_destroy.  Errors: PN_ERR_ARG, PN_ERR_WORKSPACE, PN_ERR_CUDA. */
+int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_stream, void* workspace,
+              size_t workspace_bytes);
+
+/* S0: hand the network to the library (it copies; the caller may free its arrays on return).
+ * gx, gy, gz: nx*ny*nz floats each, forward-bond convention; gz must be NULL iff nz == 1.
+ * `pointers_are_device` != 0: DEVICE pointers (device-to-device copy on the handle's stream);
+ * 0: HOST pointers (pageable or pinned).  Every in-lattice bond must be finite and >= 0, else
+ * PN_ERR_VALUE and the handle keeps no network.  Invalidates earlier pressures. */
+int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const float* gz,
+                        int pointers_are_device);
+
+/* S1..S7: classify and prune clusters for `direction` (0 = x, 1 = y, 2 = z; the axis needs >= 3
+ * node planes), then iterate until the true fp64 residual ||b - A x||_2 <= tol * ||b||_2
+ * (0 < tol < 1).  Returns when the stream work of this solve has finished.  `info` may be NULL.
+ * Returns PN_OK, PN_NO_SPANNING_CLUSTER, PN_MAX_ITERS, or an error. */
+int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info);
+
+/* Pressures of the last solve on ALL nx*ny*nz nodes (fp64, node order n = i + nx*(j + ny*k)):
+ * Dirichlet planes and pinned clusters hold their pin values.  `out`: nx*ny*nz doubles, DEVICE if
+ * `pointer_is_device` else HOST.  Valid until the next pn_solve / pn_set_conductances. */
+int pn_get_pressures(pn_ctx* ctx, double* out, int pointer_is_device);
+
+/* Node class (PN_CLASS_*) of every node for the last solve's direction; nx*ny*nz bytes. */
+int pn_get_classes(pn_ctx* ctx, signed char* out, int pointer_is_device);
+
+/* S8, eq.(4) P:61 with mu = l = 1, dP = 1, L = n_a - 1, S = number of nodes in a plane normal to a:
+ *   q_in  = sum over bonds leaving the inlet plane   g (1 - P_nbr)
+ *   q_out = sum over bonds entering the outlet plane g (P_nbr - 0)
+ *   g_eff = (q_in + q_out) / 2,   k_eff = g_eff (n_a - 1) / S.
+ * HOST pointers; any may be NULL.  Needs a finished pn_solve (PN_ERR_STATE otherwise). */
+int pn_flux(pn_ctx* ctx, double* q_in, double* q_out, double* g_eff, double* k_eff);
+
+/* Tuning knobs (PN_OPT_*).  PN_ERR_ARG on an unknown key or out-of-range value. */
+int pn_set_option(pn_ctx* ctx, int key, double value);
+
+/* Kernel launches enqueued by this handle since pn_create (bench.py's `gpu_launches`). */
+long long pn_launch_count(const pn_ctx* ctx);
+
+/* Release the handle (not the workspace).  NULL is allowed. */
+int pn_destroy(pn_ctx* ctx);
+
+/* Static text for a return code. */
+const char* pn_strerror(int code);
+
+/* Text of the last CUDA error seen by this handle ("" if none). */
+const char* pn_last_error(const pn_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PN_H */

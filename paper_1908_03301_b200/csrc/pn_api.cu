@@ -1,0 +1,440 @@
+// pn_api.cu -- the C ABI of include/pn.h: handle, workspace carving, and the host side of the
+// mixed-precision loop.  Every step of the path runs in the kernels
+// of pn_setup.cu / pn_outer.cu / pn_inner.cu; this file only sequences them and reads back a few
+// scalars per outer cycle.
+//
+// The loop ("SP inner loop ... DP outer loop", Fig.5 is a missing image; SURVEY.md 8(c) reading 4,
+// "reliable updates"):
+//   x64 = pins + initial guess;  r = b - A x64 in fp64 (S3)  ->  r_hat (fp32, scaled)
+//   repeat: fp32 CG iterations on the scaled system (S4, S5) until the recursive residual has fallen
+//           by `delta` since the last replacement, or below the proxy of the exit threshold;
+//           x64 += s * x_hat (S7, fp64);  r = b - A x64 in fp64 (S3);  exit if ||r|| <= tol ||b||;
+//           otherwise continue the SAME Krylov sequence (search direction kept, beta from the true
+//           residual) -- the fp32 solver is never restarted.
+#include <cstdio>
+#include <cstring>
+#include <cmath>
+#include <new>
+
+#include "pn_internal.cuh"
+
+struct pn_ctx {
+    int unx, uny, unz;          // user lattice
+    bool is2d;
+    pn_geom g;                  // internal lattice (direction fields filled per solve)
+    int device;
+    cudaStream_t stream;
+    char* ws;
+    size_t ws_bytes;
+    pn_ptrs P;
+    float* raw_store[3];
+    pn_state* h_state;          // pinned mirror
+    cudaEvent_t ev[4];
+    bool have_g, have_solution;
+    int last_dir_user;
+    // options
+    int max_iters, chunk, x0_linear, skip_label, variant;
+    double delta;
+    long long launches;
+    double flux[4];
+    bool flux_valid;
+    char err[256];
+};
+
+namespace {
+
+int g_sm_count = 0;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct layout {
+    pn_geom g;
+    size_t off_raw[3], off_gs[3], off_w[3], off_s, off_x64, off_r, off_p, off_p2, off_q, off_xh, off_cls, off_slots,
+        off_state, total;
+    size_t halo;                // elements in one halo plane
+};
+
+bool make_layout(int nx, int ny, int nz, layout* L) {
+    if (nx < 1 || ny < 1 || nz < 1) return false;
+    const bool is2d = (nz == 1);
+    pn_geom& g = L->g;
+    g.nx = nx;
+    g.ny = is2d ? 1 : ny;
+    g.nz = is2d ? ny : nz;
+    g.px = (nx + 3) / 4 * 4;
+    g.plane = (long long)g.px * g.ny;
+    g.npad = g.plane * g.nz;
+    g.n = (long long)nx * ny * nz;
+    g.dir = 0; g.n_a = nx; g.stride_a = 1;
+    if (g.npad + 2 * g.plane >= (1ll << 31)) return false;
+    L->halo = (size_t)g.plane;
+    const size_t vec = (size_t)g.npad + 2 * L->halo;   // elements of a padded array with its two halo planes
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
+    for (int b = 0; b < 3; ++b) L->off_raw[b] = take((size_t)g.n * 4);
+    for (int b = 0; b < 3; ++b) L->off_gs[b] = take(vec * 4);
+    for (int b = 0; b < 3; ++b) L->off_w[b] = take(vec * 4);
+    L->off_s = take(vec * 4);
+    L->off_x64 = take(vec * 8);
+    L->off_r = take(vec * 4);
+    L->off_p = take(vec * 4);
+    L->off_p2 = take(vec * 4);
+    L->off_q = take(vec * 4);
+    L->off_xh = take(vec * 4);
+    L->off_cls = take(vec);
+    L->off_slots = take(4 * PN_MAX_BLOCKS * sizeof(double));
+    L->off_state = take(sizeof(pn_state));
+    L->total = o;
+    return true;
+}
+
+struct device_guard {
+    int prev;
+    bool ok;
+    explicit device_guard(int dev) : prev(-1), ok(false) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; }
+        ok = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~device_guard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int fail_cuda(pn_ctx* c, cudaError_t e, const char* where) {
+    if (c) snprintf(c->err, sizeof(c->err), "%s: %s", where, cudaGetErrorString(e));
+    return PN_ERR_CUDA;
+}
+
+#define CK(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);     \
+    } while (0)
+
+}  // namespace
+
+int pn_sm_count() { return g_sm_count > 0 ? g_sm_count : 148; }
+
+extern "C" {
+
+size_t pn_workspace_bytes(int nx, int ny, int nz) {
+    layout L;
+    if (!make_layout(nx, ny, nz, &L)) return 0;
+    return L.total;
+}
+
+int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_stream, void* workspace,
+              size_t workspace_bytes) {
+    if (!out) return PN_ERR_ARG;
+    *out = nullptr;
+    layout L;
+    if (!make_layout(nx, ny, nz, &L)) return PN_ERR_ARG;
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < L.total) return PN_ERR_WORKSPACE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return PN_ERR_CUDA; }
+    device_guard guard(device);
+    if (!guard.ok) return PN_ERR_CUDA;
+    pn_ctx* ctx = new (std::nothrow) pn_ctx;
+    if (!ctx) return PN_ERR_ARG;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->unx = nx; ctx->uny = ny; ctx->unz = nz;
+    ctx->is2d = (nz == 1);
+    ctx->g = L.g;
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->ws = (char*)workspace;
+    ctx->ws_bytes = workspace_bytes;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0;
+    ctx->delta = 0.1;
+    ctx->last_dir_user = -1;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) g_sm_count = prop.multiProcessorCount;
+    const size_t h = L.halo;
+    pn_ptrs& P = ctx->P;
+    for (int b = 0; b < 3; ++b) {
+        ctx->raw_store[b] = (float*)(ctx->ws + L.off_raw[b]);
+        P.gs[b] = (float*)(ctx->ws + L.off_gs[b]) + h;
+        P.w[b] = (float*)(ctx->ws + L.off_w[b]) + h;
+    }
+    P.s = (float*)(ctx->ws + L.off_s) + h;
+    P.x64 = (double*)(ctx->ws + L.off_x64) + h;
+    P.r = (float*)(ctx->ws + L.off_r) + h;
+    P.p = (float*)(ctx->ws + L.off_p) + h;
+    P.p2 = (float*)(ctx->ws + L.off_p2) + h;
+    P.q = (float*)(ctx->ws + L.off_q) + h;
+    P.xh = (float*)(ctx->ws + L.off_xh) + h;
+    P.cls = (signed char*)(ctx->ws + L.off_cls) + h;
+    P.parent = (int*)P.q;
+    P.flags = (int*)P.xh;
+    P.slots = (double*)(ctx->ws + L.off_slots);
+    P.st = (pn_state*)(ctx->ws + L.off_state);
+    P.scratch = (void*)(ctx->ws + L.off_p);   // p and p2 are adjacent: 8 bytes per padded node
+    cudaError_t e = cudaMemsetAsync(ctx->ws, 0, L.total, ctx->stream);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_state, sizeof(pn_state));
+    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&ctx->ev[i]);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) {
+        if (ctx->h_state) cudaFreeHost(ctx->h_state);
+        for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+        delete ctx;
+        cudaGetLastError();
+        return PN_ERR_CUDA;
+    }
+    *out = ctx;
+    return PN_OK;
+}
+
+int pn_destroy(pn_ctx* ctx) {
+    if (!ctx) return PN_OK;
+    device_guard guard(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->h_state) cudaFreeHost(ctx->h_state);
+    for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+    return PN_OK;
+}
+
+int pn_set_option(pn_ctx* ctx, int key, double value) {
+    if (!ctx || !(value == value)) return PN_ERR_ARG;
+    switch (key) {
+        case PN_OPT_MAX_ITERS: if (value < 1 || value > 2e9) return PN_ERR_ARG; ctx->max_iters = (int)value; return PN_OK;
+        case PN_OPT_DELTA: if (!(value > 0.0 && value < 1.0)) return PN_ERR_ARG; ctx->delta = value; return PN_OK;
+        case PN_OPT_X0: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
+        case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
+        case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
+        case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
+        default: return PN_ERR_ARG;
+    }
+}
+
+long long pn_launch_count(const pn_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* pn_last_error(const pn_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+const char* pn_strerror(int code) {
+    switch (code) {
+        case PN_OK: return "ok";
+        case PN_NO_SPANNING_CLUSTER: return "no cluster spans inlet to outlet (Q = 0)";
+        case PN_MAX_ITERS: return "iteration budget spent or residual stagnated";
+        case PN_ERR_ARG: return "bad argument";
+        case PN_ERR_STATE: return "call out of order";
+        case PN_ERR_VALUE: return "conductance negative or not finite";
+        case PN_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+        case PN_ERR_CUDA: return "CUDA error";
+        case PN_ERR_BREAKDOWN: return "conjugate-gradient breakdown";
+        default: return "unknown code";
+    }
+}
+
+int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const float* gz, int pointers_are_device) {
+    if (!ctx || !gx || !gy) return PN_ERR_ARG;
+    if ((ctx->unz == 1) != (gz == nullptr)) return PN_ERR_ARG;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    ctx->have_g = false;
+    ctx->have_solution = false;
+    ctx->flux_valid = false;
+    const size_t bytes = (size_t)ctx->g.n * 4;
+    const cudaMemcpyKind kind = pointers_are_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    // internal axes: 2D lattices are held as nx x 1 x ny, so user gy feeds the internal z-bond array
+    const float* src[3] = {gx, ctx->is2d ? nullptr : gy, ctx->is2d ? gy : gz};
+    for (int b = 0; b < 3; ++b) {
+        ctx->P.raw[b] = nullptr;
+        if (!src[b]) continue;
+        CK(cudaMemcpyAsync(ctx->raw_store[b], src[b], bytes, kind, ctx->stream));
+        ctx->P.raw[b] = ctx->raw_store[b];
+    }
+    CK(cudaMemsetAsync(&ctx->P.st->bad_value, 0, 2 * sizeof(int), ctx->stream));
+    int nl = 0;
+    CK(pn_launch_validate(ctx->g, ctx->P, ctx->stream, &nl));
+    ctx->launches += nl;
+    CK(cudaMemcpyAsync(ctx->h_state, ctx->P.st, sizeof(pn_state), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (ctx->h_state->bad_value) return PN_ERR_VALUE;
+    ctx->have_g = true;
+    return PN_OK;
+}
+
+static int read_state(pn_ctx* ctx) {
+    CK(cudaMemcpyAsync(ctx->h_state, ctx->P.st, sizeof(pn_state), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PN_OK;
+}
+
+int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
+    if (info) memset(info, 0, sizeof(*info));
+    if (!ctx) return PN_ERR_ARG;
+    if (direction < 0 || direction > 2 || !(tol > 0.0 && tol < 1.0)) return PN_ERR_ARG;
+    if (ctx->is2d && direction == 2) return PN_ERR_ARG;
+    const int ulen[3] = {ctx->unx, ctx->uny, ctx->unz};
+    if (ulen[direction] < 3) return PN_ERR_ARG;
+    if (!ctx->have_g) return PN_ERR_STATE;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    ctx->have_solution = false;
+    ctx->flux_valid = false;
+    pn_geom& g = ctx->g;
+    g.dir = (ctx->is2d && direction == 1) ? 2 : direction;
+    g.n_a = ulen[direction];
+    g.stride_a = g.dir == 0 ? 1 : (g.dir == 1 ? g.px : g.plane);
+    const pn_ptrs& P = ctx->P;
+    cudaStream_t s = ctx->stream;
+    int nl = 0;
+    int rc = PN_OK;
+
+    // ---- S1 + set-up ----
+    CK(cudaEventRecord(ctx->ev[0], s));
+    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + sizeof(P.st->count), s));
+    CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
+    const bool do_label = !ctx->skip_label && ctx->h_state->any_closed;
+    CK(pn_launch_label(g, P, do_label, ctx->x0_linear, s, &nl));
+    // parent / flags aliased q / x_hat: clear the CG vectors before the first iteration
+    const size_t vbytes = (size_t)g.npad * 4;
+    CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
+    CK(cudaMemsetAsync(P.q, 0, vbytes, s));
+    // p / p2 double as export staging (pn_get_pressures), halo planes included: clear them whole
+    const size_t vhalo = ((size_t)g.npad + 2 * (size_t)g.plane) * 4;
+    CK(cudaMemsetAsync(P.p - g.plane, 0, vhalo, s));
+    CK(cudaMemsetAsync(P.p2 - g.plane, 0, vhalo, s));
+    CK(pn_launch_residual64(g, P, s, &nl));
+    CK(cudaEventRecord(ctx->ev[1], s));
+    rc = read_state(ctx);
+    if (rc) return rc;
+    pn_state* h = ctx->h_state;
+    const long long n_solved = (long long)h->count[0];
+    const double nb = sqrt(h->acc[2]);
+    double rn = sqrt(h->acc[0]);
+    double rr_hat = h->acc[1];
+    int outer = 1;
+    int status = PN_OK;
+    int total_iters = 0;
+
+    if (n_solved == 0 || !(nb > 0.0)) {
+        status = PN_NO_SPANNING_CLUSTER;
+        rn = 0.0;
+    } else if (rn > tol * nb) {
+        const double delta2 = ctx->delta * ctx->delta;
+        auto target_for = [&](double rn_true, double rr_true) {
+            // proxy of the fp64 exit test in the scaled norm: ||r|| / ||r_hat|| measured at this replacement
+            const double c = rn_true / sqrt(rr_true);
+            const double t = 0.7 * tol * nb / c;
+            return t * t;
+        };
+        CK(pn_launch_set_state(P, rr_hat, 0.0, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 1, s, &nl));
+        double best_rn = rn;
+        int stagnant = 0;
+        while (true) {
+            CK(pn_launch_inner(g, P, ctx->chunk, ctx->variant, s, &nl));
+            rc = read_state(ctx);
+            if (rc) return rc;
+            if (h->flag == PN_FLAG_RUN) continue;
+            total_iters = h->iters;
+            if (h->flag == PN_FLAG_BREAKDOWN) { status = PN_ERR_BREAKDOWN; }
+            // S7 + S3: fold the fp32 correction into x64 and recompute the true residual
+            const double rr_before = h->rr_old;   // rr entering the last iteration: beta's denominator
+            const int flag = h->flag;
+            CK(pn_launch_flush(g, P, s, &nl));
+            CK(pn_launch_residual64(g, P, s, &nl));
+            rc = read_state(ctx);
+            if (rc) return rc;
+            ++outer;
+            rn = sqrt(h->acc[0]);
+            rr_hat = h->acc[1];
+            if (status == PN_ERR_BREAKDOWN) break;
+            if (rn <= tol * nb) break;
+            if (flag == PN_FLAG_BUDGET || total_iters >= ctx->max_iters) { status = PN_MAX_ITERS; break; }
+            if (rn < 0.9 * best_rn) { best_rn = rn; stagnant = 0; }
+            else if (++stagnant >= 8) { status = PN_MAX_ITERS; break; }
+            if (!(rr_hat > 0.0)) { status = PN_MAX_ITERS; break; }
+            // continue the same Krylov sequence: beta = (true r.r) / (r.r before the last step)
+            const double beta = rr_before > 0.0 ? rr_hat / rr_before : 0.0;
+            CK(pn_launch_set_state(P, rr_hat, beta, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 0, s, &nl));
+        }
+    }
+    CK(cudaEventRecord(ctx->ev[2], s));
+    CK(cudaStreamSynchronize(s));
+    ctx->launches += nl;
+    ctx->have_solution = true;
+    ctx->last_dir_user = direction;
+    if (info) {
+        float ms = 0.f;
+        info->status = status;
+        info->outer_cycles = outer;
+        info->inner_iters = total_iters;
+        info->rel_residual = nb > 0.0 ? rn / nb : 0.0;
+        info->b_norm = nb;
+        info->n_solved = n_solved;
+        info->n_inlet_only = (long long)h->count[1];
+        info->n_outlet_only = (long long)h->count[2];
+        info->n_floating = (long long)h->count[3];
+        if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
+        if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
+    }
+    return status;
+}
+
+int pn_get_pressures(pn_ctx* ctx, double* out, int pointer_is_device) {
+    if (!ctx || !out) return PN_ERR_ARG;
+    if (!ctx->have_solution) return PN_ERR_STATE;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    const pn_geom& g = ctx->g;
+    const size_t bytes = (size_t)g.n * sizeof(double);
+    int nl = 0;
+    if (g.px == g.nx) {   // padded layout == user layout
+        CK(cudaMemcpyAsync(out, ctx->P.x64, bytes, pointer_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    } else if (pointer_is_device) {
+        CK(pn_launch_export_x(g, ctx->P, out, ctx->stream, &nl));
+    } else {
+        CK(pn_launch_export_x(g, ctx->P, (double*)ctx->P.scratch, ctx->stream, &nl));
+        CK(cudaMemcpyAsync(out, ctx->P.scratch, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    ctx->launches += nl;
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PN_OK;
+}
+
+int pn_get_classes(pn_ctx* ctx, signed char* out, int pointer_is_device) {
+    if (!ctx || !out) return PN_ERR_ARG;
+    if (!ctx->have_solution) return PN_ERR_STATE;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    const pn_geom& g = ctx->g;
+    int nl = 0;
+    if (pointer_is_device) {
+        CK(pn_launch_export_cls(g, ctx->P, out, 0, ctx->stream, &nl));
+    } else {
+        CK(pn_launch_export_cls(g, ctx->P, (signed char*)ctx->P.scratch, 0, ctx->stream, &nl));
+        CK(cudaMemcpyAsync(out, ctx->P.scratch, (size_t)g.n, cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    ctx->launches += nl;
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PN_OK;
+}
+
+int pn_flux(pn_ctx* ctx, double* q_in, double* q_out, double* g_eff, double* k_eff) {
+    if (!ctx) return PN_ERR_ARG;
+    if (!ctx->have_solution) return PN_ERR_STATE;
+    if (!ctx->flux_valid) {   // S8: one fused kernel over the two boundary planes, four scalars back
+        device_guard guard(ctx->device);
+        if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+        const pn_geom& g = ctx->g;
+        int nl = 0;
+        CK(pn_launch_flux(g, ctx->P, ctx->stream, &nl));
+        ctx->launches += nl;
+        int rc = read_state(ctx);
+        if (rc) return rc;
+        const double qi = ctx->h_state->acc[0], qo = ctx->h_state->acc[1];
+        const long long s_perp = g.n / g.n_a;
+        ctx->flux[0] = qi;
+        ctx->flux[1] = qo;
+        ctx->flux[2] = 0.5 * (qi + qo);
+        ctx->flux[3] = ctx->flux[2] * (double)(g.n_a - 1) / (double)s_perp;
+        ctx->flux_valid = true;
+    }
+    if (q_in) *q_in = ctx->flux[0];
+    if (q_out) *q_out = ctx->flux[1];
+    if (g_eff) *g_eff = ctx->flux[2];
+    if (k_eff) *k_eff = ctx->flux[3];
+    return PN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,163 @@
+// pn_inner.cu -- the fp32 inner conjugate-gradient iteration: two fused
+// kernels per iteration, all scalars device-resident.
+//
+// Paper: K2 "sparse matrix-vector multiplication ... each Z_i multiplied by its P_i, block reduction"
+// (P:89), K3 "a thread is assigned for the calculation of each element of U, R and Z ... partial
+// result of dot products", "Merging the calculations of the vectors' entries into a single
+// kernel ... decreasing the number of times that the global memory must be accessed", final
+// sums of the 2^6 block partials on the CPU.  Here: matrix-free 7-point operator, the final
+// sums stay on the device (last-block-done), and the Jacobi preconditioner (north_star (b)) is
+// applied as the symmetric scaling A_hat = D^-1/2 A D^-1/2 folded into one fp32 weight per bond,
+//     w_ij = g_ij / sqrt(d_i d_j),   A_hat = I - W,
+// so that Jacobi-PCG on A is plain CG on A_hat (same iterates in exact arithmetic) and the unit
+// diagonal costs no memory traffic.  Nodes that are not unknowns (Dirichlet planes, pinned clusters,
+// pad columns) have all their weights zero and r = p = 0, so they need no mask.
+//
+// Iteration t (state.iters == t), p double-buffered because kernel A reads neighbours' old p:
+//   kernel A:  p_new = r + beta p_old          (at the node AND its six neighbours, recomputed)
+//              x_hat += alpha_x p_old          (the solution update of iteration t-1, deferred)
+//              q = p_new - W p_new ;  pq = p_new . q     -> alpha = rr / pq       (last block)
+//   kernel B:  r -= alpha q ;  rr' = r . r     -> beta = rr'/rr, alpha_x = alpha, flags (last block)
+// Bytes per node-iteration (3D): A reads r, p, x_hat, wx, wy, wz (24) writes p, q, x_hat (12);
+// B reads r, q (8) writes r (4): 48 B.
+#include "pn_internal.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ void st4(float* p, const float4& v) { *reinterpret_cast<float4*>(p) = v; }
+__device__ __forceinline__ float4 fma4(float a, const float4& x, const float4& y) {
+    return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
+}
+
+// Last-block epilogue of kernel A: alpha = rr / (p.Ap); breakdown guards.
+__device__ __forceinline__ void finish_A(pn_state* st, double pq) {
+    st->pq = pq;
+    if (st->rr == 0.0) st->flag = PN_FLAG_CONVERGED;
+    else if (!(pq > 0.0) || isinf(pq)) st->flag = PN_FLAG_BREAKDOWN;
+    else st->alpha = st->rr / pq;
+}
+
+// Last-block epilogue of kernel B: beta, bookkeeping, and the triggers the host polls for.
+__device__ __forceinline__ void finish_B(pn_state* st, double rr_new) {
+    const double rr_old = st->rr;
+    st->rr_old = rr_old;
+    st->rr = rr_new;
+    st->beta = rr_new / rr_old;
+    st->alpha_x = st->alpha;
+    const int it = st->iters + 1;
+    st->iters = it;
+    double rr_max = st->rr_max;
+    if (rr_new > rr_max) { rr_max = rr_new; st->rr_max = rr_max; }
+    if (!(rr_new >= 0.0) || isinf(rr_new)) st->flag = PN_FLAG_BREAKDOWN;
+    else if (rr_new <= st->rr_target) st->flag = PN_FLAG_CONVERGED;
+    else if (rr_new < st->delta2 * rr_max) st->flag = PN_FLAG_UPDATE;
+    else if (it >= st->max_iters) st->flag = PN_FLAG_BUDGET;
+}
+
+// ---- kernel A, reference variant: one thread per 4 consecutive nodes, neighbours through L1/L2 ---
+__global__ void __launch_bounds__(TPB) k_stencil_simple(int nvec, int px, int plane, pn_ptrs P, float* p0, float* p1) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;
+    __shared__ double sm[32];
+    __shared__ double tot[1];
+    const float beta = (float)st->beta;
+    const float ax = (float)st->alpha_x;
+    const int par = st->iters & 1;
+    const float* __restrict__ pin = par ? p1 : p0;
+    float* __restrict__ pout = par ? p0 : p1;
+    const float* __restrict__ r = P.r;
+    const float* __restrict__ wx = P.w[0];
+    const float* __restrict__ wy = P.w[1];
+    const float* __restrict__ wz = P.w[2];
+    double acc = 0.0;
+    for (int v = blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += gridDim.x * blockDim.x) {
+        const long long n = 4ll * v;
+        const float4 pc = ld4(pin + n);
+        const float4 pn = fma4(beta, pc, ld4(r + n));
+        st4(P.xh + n, fma4(ax, pc, ld4(P.xh + n)));
+        const float pl = fmaf(beta, pin[n - 1], r[n - 1]);
+        const float pr = fmaf(beta, pin[n + 4], r[n + 4]);
+        const float4 pym = fma4(beta, ld4(pin + n - px), ld4(r + n - px));
+        const float4 pyp = fma4(beta, ld4(pin + n + px), ld4(r + n + px));
+        const float4 pzm = fma4(beta, ld4(pin + n - plane), ld4(r + n - plane));
+        const float4 pzp = fma4(beta, ld4(pin + n + plane), ld4(r + n + plane));
+        const float4 gx = ld4(wx + n), gy = ld4(wy + n), gz = ld4(wz + n);
+        const float gxl = wx[n - 1];
+        const float4 gym = ld4(wy + n - px), gzm = ld4(wz + n - plane);
+        float4 q;
+        q.x = pn.x - (gxl * pl + gx.x * pn.y + gym.x * pym.x + gy.x * pyp.x + gzm.x * pzm.x + gz.x * pzp.x);
+        q.y = pn.y - (gx.x * pn.x + gx.y * pn.z + gym.y * pym.y + gy.y * pyp.y + gzm.y * pzm.y + gz.y * pzp.y);
+        q.z = pn.z - (gx.y * pn.y + gx.z * pn.w + gym.z * pym.z + gy.z * pyp.z + gzm.z * pzm.z + gz.z * pzp.z);
+        q.w = pn.w - (gx.z * pn.z + gx.w * pr + gym.w * pym.w + gy.w * pyp.w + gzm.w * pzm.w + gz.w * pzp.w);
+        st4(pout + n, pn);
+        st4(P.q + n, q);
+        acc += (double)(pn.x * q.x + pn.y * q.y + pn.z * q.z + pn.w * q.w);
+    }
+    acc = pn_block_sum(acc, sm);
+    const double v1[1] = {acc};
+    if (pn_grid_sum<1>(v1, P.slots, &st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) finish_A(st, tot[0]);
+    }
+}
+
+// ---- kernel B: r -= alpha q, rr = r.r  (a pure stream: 12 B per node) ---------------------------
+__global__ void __launch_bounds__(TPB) k_update(int nvec, pn_ptrs P) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;
+    __shared__ double sm[32];
+    __shared__ double tot[1];
+    const float nalpha = -(float)st->alpha;
+    float* __restrict__ r = P.r;
+    const float* __restrict__ q = P.q;
+    double acc = 0.0;
+    const int stride = gridDim.x * blockDim.x;
+    int v = blockIdx.x * blockDim.x + threadIdx.x;
+    for (; v + 3 * stride < nvec; v += 4 * stride) {   // four independent 16-byte loads per array in flight
+        float4 a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = ld4(r + 4ll * (v + u * stride)); b[u] = __ldcs(reinterpret_cast<const float4*>(q + 4ll * (v + u * stride))); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float4 t = fma4(nalpha, b[u], a[u]);
+            st4(r + 4ll * (v + u * stride), t);
+            acc += (double)(t.x * t.x + t.y * t.y + t.z * t.z + t.w * t.w);
+        }
+    }
+    for (; v < nvec; v += stride) {
+        const float4 t = fma4(nalpha, ld4(q + 4ll * v), ld4(r + 4ll * v));
+        st4(r + 4ll * v, t);
+        acc += (double)(t.x * t.x + t.y * t.y + t.z * t.z + t.w * t.w);
+    }
+    acc = pn_block_sum(acc, sm);
+    const double v1[1] = {acc};
+    if (pn_grid_sum<1>(v1, P.slots, &st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) finish_B(st, tot[0]);
+    }
+}
+
+int grid_for(long long work_items) {
+    long long nb = (work_items + TPB - 1) / TPB;
+    long long cap = (long long)pn_sm_count() * 8;
+    if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
+    if (nb > cap) nb = cap;
+    if (nb < 1) nb = 1;
+    return (int)nb;
+}
+
+}  // namespace
+
+cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int variant, cudaStream_t st,
+                            int* launches) {
+    const int nvec = (int)(g.npad / 4);
+    const int nb = grid_for(nvec);
+    (void)variant;
+    for (int it = 0; it < iterations; ++it) {
+        k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2);
+        k_update<<<nb, TPB, 0, st>>>(nvec, P);
+    }
+    *launches += 2 * iterations;
+    return cudaGetLastError();
+}

@@ -1,0 +1,160 @@
+// pn_outer.cu -- the double-precision outer loop, the boundary flux (S8) and
+// the export kernels.
+//
+// "...iterations with the DP are used to converge to the final solution within the allowed
+// error of the outer loop".  Here (north_star (c)): fp64 true residual r = b - A x with A applied
+// matrix-free from the fp32 conductances widened exactly, the diagonal summed on the fly in fp64;
+// the residual is handed to the fp32 inner CG in the symmetric-Jacobi-scaled variables
+// (r_hat = s r, s = diag^-1/2), and the fp32 correction comes back as x += s * x_hat.
+#include "pn_internal.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+
+int grid_for(long long work_items) {
+    long long nb = (work_items + TPB - 1) / TPB;
+    long long cap = (long long)pn_sm_count() * 8;
+    if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
+    if (nb > cap) nb = cap;
+    if (nb < 1) nb = 1;
+    return (int)nb;
+}
+
+// ---- S3: r = b - A x in fp64 on solved nodes, written as r_hat = (float)(s r) -------------------
+// x64 carries the Dirichlet and pin values on the nodes that are not unknowns, so
+// (b - A x)_i = sum_j g_ij (x_j - x_i) over all six neighbours.  acc[0] = ||r||^2, acc[1] = ||r_hat||^2
+// (of the rounded fp32 values, i.e. exactly what the inner recurrence starts from).
+__global__ void k_residual64(pn_geom g, pn_ptrs P) {
+    __shared__ double sm[32];
+    __shared__ double tot[2];
+    double a0 = 0.0, a1 = 0.0;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const float s = P.s[n];
+        float rh = 0.f;
+        if (s != 0.f) {
+            const double xc = P.x64[n];
+            double r = (double)P.gs[0][n] * (P.x64[n + 1] - xc);
+            r += (double)P.gs[0][n - 1] * (P.x64[n - 1] - xc);
+            r += (double)P.gs[1][n] * (P.x64[n + g.px] - xc);
+            r += (double)P.gs[1][n - g.px] * (P.x64[n - g.px] - xc);
+            r += (double)P.gs[2][n] * (P.x64[n + g.plane] - xc);
+            r += (double)P.gs[2][n - g.plane] * (P.x64[n - g.plane] - xc);
+            rh = (float)((double)s * r);
+            a0 += r * r;
+            a1 += (double)rh * (double)rh;
+        }
+        P.r[n] = rh;
+    }
+    a0 = pn_block_sum(a0, sm);
+    a1 = pn_block_sum(a1, sm);
+    const double v[2] = {a0, a1};
+    if (pn_grid_sum<2>(v, P.slots, &P.st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) { P.st->acc[0] = tot[0]; P.st->acc[1] = tot[1]; }
+    }
+}
+
+// ---- S7: x64 += s * (x_hat + alpha_x p)  (the pending deferred update included); x_hat = 0 ------
+__global__ void k_flush(pn_geom g, pn_ptrs P) {
+    const double ax = P.st->alpha_x;
+    const float* __restrict__ p = (P.st->iters & 1) ? P.p2 : P.p;   // the direction of the last iteration
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const float s = P.s[n];
+        if (s != 0.f) P.x64[n] += (double)s * ((double)P.xh[n] + ax * (double)p[n]);
+        P.xh[n] = 0.f;
+    }
+}
+
+__global__ void k_set_state(pn_state* st, double rr, double beta, double rr_max, double rr_target, double delta2,
+                            int max_iters, int reset_iters) {
+    st->rr = rr;
+    st->rr_old = rr;
+    st->beta = beta;
+    st->alpha = 0.0;
+    st->alpha_x = 0.0;
+    st->pq = 0.0;
+    st->rr_max = rr_max;
+    st->rr_target = rr_target;
+    st->delta2 = delta2;
+    st->max_iters = max_iters;
+    if (reset_iters) st->iters = 0;
+    st->flag = PN_FLAG_RUN;
+    st->ticket = 0u;
+}
+
+// ---- S8: boundary fluxes, eq.(4) P:61.  acc[0] = Q_in, acc[1] = Q_out ---------------------------
+// One thread per node of a plane normal to the solve axis; the solve copy of g has every bond of a
+// pinned node zeroed, so summing over ALL boundary bonds is exact (SURVEY.md 8(a) note on S1/S8).
+__global__ void k_flux(pn_geom g, pn_ptrs P) {
+    __shared__ double sm[32];
+    __shared__ double tot[2];
+    const int d0 = g.dir == 0 ? g.ny : g.nx;                       // fast in-plane extent
+    const int d1 = g.dir == 2 ? g.ny : g.nz;                       // slow in-plane extent
+    const long long s0 = g.dir == 0 ? g.px : 1;                    // their element strides
+    const long long s1 = g.dir == 2 ? g.px : g.plane;
+    const long long m = (long long)d0 * d1;
+    double qi = 0.0, qo = 0.0;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < m; t += (long long)gridDim.x * blockDim.x) {
+        const long long base = (t % d0) * s0 + (t / d0) * s1;
+        const long long n_in = base;                                // node on the inlet plane
+        const long long n_out = base + (long long)(g.n_a - 2) * g.stride_a;  // node next to the outlet plane
+        qi += (double)P.gs[g.dir][n_in] * (P.x64[n_in] - P.x64[n_in + g.stride_a]);
+        qo += (double)P.gs[g.dir][n_out] * (P.x64[n_out] - P.x64[n_out + g.stride_a]);
+    }
+    qi = pn_block_sum(qi, sm);
+    qo = pn_block_sum(qo, sm);
+    const double v[2] = {qi, qo};
+    if (pn_grid_sum<2>(v, P.slots, &P.st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) { P.st->acc[0] = tot[0]; P.st->acc[1] = tot[1]; }
+    }
+}
+
+// ---- padded -> user layout ----------------------------------------------------------------------
+__global__ void k_export_x(pn_geom g, const double* __restrict__ x64, double* __restrict__ out) {
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.n; n += (long long)gridDim.x * blockDim.x) {
+        const long long row = n / g.nx;
+        out[n] = x64[row * g.px + (n - row * g.nx)];
+    }
+}
+__global__ void k_export_cls(pn_geom g, const signed char* __restrict__ cls, signed char* __restrict__ out) {
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.n; n += (long long)gridDim.x * blockDim.x) {
+        const long long row = n / g.nx;
+        out[n] = cls[row * g.px + (n - row * g.nx)];
+    }
+}
+
+}  // namespace
+
+cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    k_residual64<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    k_flush<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,
+                                double delta2, int max_iters, int reset_iters, cudaStream_t st, int* launches) {
+    k_set_state<<<1, 1, 0, st>>>(P.st, rr, beta, rr_max, rr_target, delta2, max_iters, reset_iters);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_flux(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    const long long m = g.n / g.n_a;
+    k_flux<<<grid_for(m), TPB, 0, st>>>(g, P);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_export_x(const pn_geom& g, const pn_ptrs& P, double* out, cudaStream_t st, int* launches) {
+    k_export_x<<<grid_for(g.n), TPB, 0, st>>>(g, P.x64, out);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_export_cls(const pn_geom& g, const pn_ptrs& P, signed char* out, int, cudaStream_t st,
+                                 int* launches) {
+    k_export_cls<<<grid_for(g.n), TPB, 0, st>>>(g, P.cls, out);
+    ++*launches;
+    return cudaGetLastError();
+}

@@ -1,0 +1,256 @@
+// pn_setup.cu -- S0 validation and S1 "classify & prune", plus the per-direction
+// set-up of the scaled inner system.  Integer / fp64 work done once per solve; not the hot loop.
+//
+// S1 is not in the paper (it never says how isolated clusters are handled, P:111, P:132 only note the
+// critical slow-down); BASELINE.json's north_star mandates it: "Dead-end and isolated clusters ... are
+// removed before the solve by a connectivity labelling pass, and their rows are pinned."  Classes
+// follow SURVEY.md 8(c) steps 2-3.  The labelling is a lock-free union-find over the interior nodes
+// (hook the larger root under the smaller with atomicCAS, path halving on find); the oracle uses a
+// serial BFS, so the two share nothing but the definition of a component.
+#include "pn_internal.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+
+__host__ __device__ inline long long cdiv(long long a, long long b) { return (a + b - 1) / b; }
+
+int grid_for(long long work_items) {
+    long long nb = cdiv(work_items, TPB);
+    long long cap = (long long)pn_sm_count() * 8;
+    if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
+    if (nb > cap) nb = cap;
+    if (nb < 1) nb = 1;
+    return (int)nb;
+}
+
+// ---- S0: every in-lattice bond finite and >= 0; note whether any is closed ----------------------
+__global__ void k_validate(pn_geom g, const float* __restrict__ r0, const float* __restrict__ r1,
+                           const float* __restrict__ r2, pn_state* st) {
+    int bad = 0, closed = 0;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.n; n += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(n % g.nx), j = (int)((n / g.nx) % g.ny), k = (int)(n / ((long long)g.nx * g.ny));
+        if (i + 1 < g.nx) { const float v = r0[n]; bad |= !(v >= 0.0f) || isinf(v); closed |= (v == 0.0f); }
+        if (r1 && j + 1 < g.ny) { const float v = r1[n]; bad |= !(v >= 0.0f) || isinf(v); closed |= (v == 0.0f); }
+        if (r2 && k + 1 < g.nz) { const float v = r2[n]; bad |= !(v >= 0.0f) || isinf(v); closed |= (v == 0.0f); }
+    }
+    bad = __syncthreads_or(bad);
+    closed = __syncthreads_or(closed);
+    if (threadIdx.x == 0) {
+        if (bad) atomicOr(&st->bad_value, 1);
+        if (closed) atomicOr(&st->any_closed, 1);
+    }
+}
+
+struct coords { int i, j, k; };
+__device__ __forceinline__ coords coords_of(const pn_geom& g, long long n) {
+    coords c;
+    c.i = (int)(n % g.px);
+    c.j = (int)((n / g.px) % g.ny);
+    c.k = (int)(n / g.plane);
+    return c;
+}
+__device__ __forceinline__ int along(const pn_geom& g, const coords& c) { return g.dir == 0 ? c.i : (g.dir == 1 ? c.j : c.k); }
+
+// ---- S1a: solve copy of g in the padded layout; union-find forest initialised -------------------
+// Off-lattice forward entries and pad columns -> 0.  Bonds lying INSIDE a Dirichlet plane (both ends
+// at the same fixed pressure, no current) -> 0.
+__global__ void k_solve_copy(pn_geom g, pn_ptrs P) {
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const coords c = coords_of(g, n);
+        float v[3] = {0.f, 0.f, 0.f};
+        if (c.i < g.nx) {
+            const long long nu = c.i + (long long)g.nx * (c.j + (long long)g.ny * c.k);
+            const int ca = along(g, c);
+            const bool dirichlet = (ca == 0) || (ca == g.n_a - 1);
+            const bool in0 = c.i + 1 < g.nx, in1 = c.j + 1 < g.ny, in2 = c.k + 1 < g.nz;
+            if (in0 && !(dirichlet && g.dir != 0)) v[0] = P.raw[0][nu];
+            if (in1 && P.raw[1] && !(dirichlet && g.dir != 1)) v[1] = P.raw[1][nu];
+            if (in2 && P.raw[2] && !(dirichlet && g.dir != 2)) v[2] = P.raw[2][nu];
+        }
+        P.gs[0][n] = v[0];
+        P.gs[1][n] = v[1];
+        P.gs[2][n] = v[2];
+        P.parent[n] = (int)n;
+        P.flags[n] = 0;
+    }
+}
+
+// ---- union-find primitives (parent[] read at L2: another SM may have just re-hooked a root) -----
+__device__ __forceinline__ int uf_find(int* parent, int x) {
+    int p = __ldcg(parent + x);
+    while (p != x) {
+        const int gp = __ldcg(parent + p);
+        if (gp != p) parent[x] = gp;  // path halving; benign race: gp is an ancestor of x
+        x = p;
+        p = gp;
+    }
+    return x;
+}
+__device__ __forceinline__ void uf_union(int* parent, int a, int b) {
+    while (true) {
+        a = uf_find(parent, a);
+        b = uf_find(parent, b);
+        if (a == b) return;
+        if (a < b) { const int t = a; a = b; b = t; }
+        const int old = atomicCAS(parent + a, a, b);  // hook the larger root under the smaller
+        if (old == a) return;
+        a = old;  // a stopped being a root meanwhile: carry on from its new parent
+    }
+}
+
+// ---- S1b: unite interior nodes joined by an open bond -------------------------------------------
+__global__ void k_union(pn_geom g, pn_ptrs P) {
+    const long long stride[3] = {1, g.px, g.plane};
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const coords c = coords_of(g, n);
+        if (c.i >= g.nx) continue;
+        const int ca = along(g, c);
+        if (ca == 0 || ca == g.n_a - 1) continue;  // Dirichlet nodes are not part of any cluster
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            if (!(P.gs[b][n] > 0.f)) continue;
+            if (b == g.dir && ca + 1 == g.n_a - 1) continue;  // forward neighbour is an outlet node
+            uf_union(P.parent, (int)n, (int)(n + stride[b]));
+        }
+    }
+}
+
+// ---- S1c: which clusters touch the inlet / outlet plane through an open bond --------------------
+__global__ void k_touch(pn_geom g, pn_ptrs P) {
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const coords c = coords_of(g, n);
+        if (c.i >= g.nx) continue;
+        const int ca = along(g, c);
+        if (ca == 0 || ca == g.n_a - 1) continue;
+        const int root = uf_find(P.parent, (int)n);
+        P.parent[n] = root;
+        int t = 0;
+        if (ca == 1 && P.gs[g.dir][n - g.stride_a] > 0.f) t |= 1;          // open bond to the inlet plane
+        if (ca == g.n_a - 2 && P.gs[g.dir][n] > 0.f) t |= 2;               // open bond to the outlet plane
+        if (t) atomicOr(P.flags + root, t);
+    }
+}
+
+// ---- S1d: node classes, class counts, pin values and the initial guess --------------------------
+template <bool LABEL>
+__global__ void k_classify(pn_geom g, pn_ptrs P, int x0_linear) {
+    unsigned long long cnt[4] = {0, 0, 0, 0};
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const coords c = coords_of(g, n);
+        int cls = PN_CLASS_PAD;
+        double x = 0.0;
+        if (c.i < g.nx) {
+            const int ca = along(g, c);
+            if (ca == 0) { cls = PN_CLASS_INLET; x = 1.0; }
+            else if (ca == g.n_a - 1) { cls = PN_CLASS_OUTLET; }
+            else {
+                int f = 3;
+                if (LABEL) f = __ldcg(P.flags + uf_find(P.parent, (int)n));
+                if (f == 3) { cls = PN_CLASS_SOLVED; x = x0_linear ? 1.0 - (double)ca / (double)(g.n_a - 1) : 0.0; cnt[0]++; }
+                else if (f == 1) { cls = PN_CLASS_INLET_ONLY; x = 1.0; cnt[1]++; }
+                else if (f == 2) { cls = PN_CLASS_OUTLET_ONLY; cnt[2]++; }
+                else { cls = PN_CLASS_FLOATING; cnt[3]++; }
+            }
+        }
+        P.cls[n] = (signed char)cls;
+        P.x64[n] = x;
+    }
+    __shared__ unsigned long long sc[4];
+    if (threadIdx.x < 4) sc[threadIdx.x] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        unsigned long long v = cnt[q];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0 && v) atomicAdd(&sc[q], v);
+    }
+    __syncthreads();
+    if (threadIdx.x < 4 && sc[threadIdx.x]) atomicAdd(&P.st->count[threadIdx.x], sc[threadIdx.x]);
+}
+
+// ---- S1e: prune -- zero every bond that has a pinned end (pinned rows get a zero diagonal) ------
+__global__ void k_prune(pn_geom g, pn_ptrs P) {
+    const long long stride[3] = {1, g.px, g.plane};
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const int c0 = P.cls[n];
+        const bool keep0 = c0 <= PN_CLASS_SOLVED;
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const float v = P.gs[b][n];
+            if (v == 0.f) continue;
+            // v != 0 implies the forward neighbour is a real node (off-lattice entries were zeroed)
+            const bool keep1 = P.cls[n + stride[b]] <= PN_CLASS_SOLVED;
+            if (!(keep0 && keep1)) P.gs[b][n] = 0.f;
+        }
+    }
+}
+
+// ---- diagonal (on the fly, fp64) -> symmetric Jacobi scale s = 1/sqrt(diag); ||b||^2 -----------
+// b_i = sum over inlet-plane neighbours of g_ij * 1 ("b is a vector related to the external
+// boundary conditions"); only nodes on the plane coord_a = 1 have one.
+__global__ void k_scale(pn_geom g, pn_ptrs P) {
+    __shared__ double sm[32];
+    __shared__ double tot[1];
+    double bb = 0.0;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        float s = 0.f;
+        if (P.cls[n] == PN_CLASS_SOLVED) {
+            const double d = (double)P.gs[0][n] + (double)P.gs[0][n - 1] + (double)P.gs[1][n] + (double)P.gs[1][n - g.px] +
+                             (double)P.gs[2][n] + (double)P.gs[2][n - g.plane];
+            s = d > 0.0 ? (float)(1.0 / sqrt(d)) : 0.f;
+            const coords c = coords_of(g, n);
+            if (along(g, c) == 1) { const double b = (double)P.gs[g.dir][n - g.stride_a]; bb += b * b; }
+        }
+        P.s[n] = s;
+    }
+    bb = pn_block_sum(bb, sm);
+    const double v[1] = {bb};
+    if (pn_grid_sum<1>(v, P.slots, &P.st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) P.st->acc[2] = tot[0];
+    }
+}
+
+// ---- scaled bond weights of the inner system: w_ij = g_ij s_i s_j (fp64 product, rounded once) --
+__global__ void k_weights(pn_geom g, pn_ptrs P) {
+    const long long stride[3] = {1, g.px, g.plane};
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const double s0 = (double)P.s[n];
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const double v = (double)P.gs[b][n];
+            float w = 0.f;
+            if (v != 0.0 && s0 != 0.0) w = (float)(v * s0 * (double)P.s[n + stride[b]]);
+            P.w[b][n] = w;
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    k_validate<<<grid_for(g.n), TPB, 0, st>>>(g, P.raw[0], P.raw[1], P.raw[2], P.st);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, int x0_linear, cudaStream_t st,
+                            int* launches) {
+    const int nb = grid_for(g.npad);
+    k_solve_copy<<<nb, TPB, 0, st>>>(g, P);
+    ++*launches;
+    if (do_label) {
+        k_union<<<nb, TPB, 0, st>>>(g, P);
+        k_touch<<<nb, TPB, 0, st>>>(g, P);
+        k_classify<true><<<nb, TPB, 0, st>>>(g, P, x0_linear);
+        k_prune<<<nb, TPB, 0, st>>>(g, P);
+        *launches += 4;
+    } else {
+        k_classify<false><<<nb, TPB, 0, st>>>(g, P, x0_linear);
+        ++*launches;
+    }
+    k_scale<<<nb, TPB, 0, st>>>(g, P);
+    k_weights<<<nb, TPB, 0, st>>>(g, P);
+    *launches += 2;
+    return cudaGetLastError();
+}

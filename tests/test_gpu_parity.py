@@ -1,0 +1,306 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the fp64 CPU oracle,
+element by element on the same seeded inputs.
+
+Tolerances are BASELINE.json's north_star: relative L_inf error 1e-8 in node pressures (max |P| = 1,
+so absolute), 1e-9 in effective conductance.  Node classes (integer work) must match bit for bit.
+Parity solves use tol = 1e-12 (1e-13 from 128^3 up): a 1e-10 residual does not imply 1e-8 in
+pressure on the diluted networks (SURVEY.md 8(c) consequence (ii)); timing runs use 1e-10.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+P_TOL = 1e-8
+G_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def pn():
+    from paper_1908_03301_b200 import build, pn as _pn
+    build.build()
+    _pn.load_library()
+    return _pn
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import c_oracle
+    c_oracle.build()
+    return c_oracle
+
+
+def gpu_solve(pn, net, direction, tol, opts=None):
+    h = pn.Network(net.nx, net.ny, net.nz)
+    for k, v in (opts or {}).items():
+        h.set_option(k, v)
+    h.set_conductances(net.gx, net.gy, net.gz)
+    info = h.solve(direction, tol, accept=(pn.PN_OK, pn.PN_NO_SPANNING_CLUSTER, pn.PN_MAX_ITERS))
+    P = h.pressures().cpu().numpy()
+    cls = h.classes().cpu().numpy()
+    fl = h.flux()
+    n_launch = h.launch_count()
+    h.close()
+    return info, P, cls, fl, n_launch
+
+
+def compare(pn, oracle, net, direction, tol=1e-12, opts=None):
+    ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13)
+    info, P, cls, fl, n_launch = gpu_solve(pn, net, direction, tol, opts)
+    assert n_launch > 0
+    # integer work: classes bit-exact, counts equal
+    assert np.array_equal(cls, ref.classes), "node classes differ from the oracle's serial BFS"
+    assert (info.n_solved, info.n_inlet_only, info.n_outlet_only, info.n_floating) == \
+        (ref.n_solved, ref.n_inlet_only, ref.n_outlet_only, ref.n_floating)
+    if ref.status == "no_spanning_cluster":
+        assert info.status == pn.PN_NO_SPANNING_CLUSTER
+        assert fl[0] == 0.0 and fl[1] == 0.0 and fl[2] == 0.0
+        assert np.array_equal(P, ref.P)
+        return info, P, fl, ref
+    assert info.status == pn.PN_OK, f"status {info.status}, residual {info.rel_residual}"
+    assert info.rel_residual <= tol
+    assert ref.rel_residual <= 2e-13
+    err = float(np.max(np.abs(P - ref.P)))
+    assert err <= P_TOL, f"pressure L_inf error {err:.3e}"
+    gerr = abs(fl[2] - ref.g_eff) / abs(ref.g_eff)
+    assert gerr <= G_TOL, f"G_eff relative error {gerr:.3e}"
+    assert abs(fl[0] - ref.q_in) <= 1e-8 * abs(ref.q_in)
+    assert abs(fl[1] - ref.q_out) <= 1e-8 * abs(ref.q_out)
+    n_a = (net.nx, net.ny, net.nz)[direction]
+    s_perp = net.n_nodes // n_a
+    assert fl[3] == pytest.approx(fl[2] * (n_a - 1) / s_perp, rel=1e-14)
+    return info, P, fl, ref
+
+
+# ---- the five configs (CFG1 full size; scaled-down siblings of CFG2..5) ---------------------------
+def test_cfg1_full(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    info, *_ = compare(pn, oracle, inputs.cfg1_iid_2d(), 0)
+    assert info.inner_iters > 0 and info.outer_cycles >= 2
+
+
+def test_cfg2_sibling(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg2_fbm_2d(256, 256), 0)
+
+
+def test_cfg3_sibling(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    info, *_ = compare(pn, oracle, inputs.cfg3_percolation_3d(48, 48, 48), 0)
+    assert info.n_floating > 0 and info.n_solved > 0
+
+
+def test_cfg4_sibling(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(64, 64, 64), 0)
+
+
+@pytest.mark.parametrize("direction", [0, 2])
+def test_cfg5_sibling(pn, oracle, direction):
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg5_stratified_3d(48, 48, 48), direction)
+
+
+def test_cfg4_sibling_128(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13)
+
+
+# ---- ragged shapes, every direction, 2D and 3D, with and without dilution ------------------------
+@pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 31, 7), (130, 6, 3)])
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("p", [1.0, 0.6])
+def test_ragged_3d(pn, oracle, shape, direction, p):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(*shape, seed=7 + direction, p=p)
+    compare(pn, oracle, net, direction)
+
+
+@pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (3, 64), (257, 31)])
+@pytest.mark.parametrize("direction", [0, 1])
+@pytest.mark.parametrize("p", [1.0, 0.7])
+def test_ragged_2d(pn, oracle, shape, direction, p):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(shape[0], shape[1], 1, seed=11 + direction, p=p)
+    compare(pn, oracle, net, direction)
+
+
+def test_reference_kernel_variant(pn, oracle):
+    """The reference stencil kernel (PN_OPT_KERNEL = 1) must pass the same parity bar."""
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(40, 36, 33), 0, opts={pn.PN_OPT_KERNEL: 1})
+    compare(pn, oracle, inputs.cfg1_iid_2d(), 0, opts={pn.PN_OPT_KERNEL: 1})
+
+
+def test_zero_start_and_restart_options(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg3_percolation_3d(32, 32, 32)
+    compare(pn, oracle, net, 0, opts={pn.PN_OPT_X0: 0})
+    compare(pn, oracle, net, 0, opts={pn.PN_OPT_DELTA: 0.01, pn.PN_OPT_CHUNK: 7})
+
+
+# ---- closed forms straight on the GPU path (also pins of the oracle, see test_oracle_pins.py) ----
+@pytest.mark.parametrize("direction", [0, 1, 2])
+def test_uniform_closed_form(pn, direction):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.uniform(9, 6, 5, 0.37)
+    info, P, cls, fl, _ = gpu_solve(pn, net, direction, 1e-12)
+    n_a = (9, 6, 5)[direction]
+    s_perp = 9 * 6 * 5 // n_a
+    assert fl[2] == pytest.approx(np.float64(np.float32(0.37)) * s_perp / (n_a - 1), rel=1e-12)
+    assert fl[3] == pytest.approx(np.float64(np.float32(0.37)), rel=1e-12)
+    c = np.arange(n_a) / (n_a - 1.0)
+    shape = [1, 1, 1]
+    shape[2 - direction] = n_a
+    assert np.max(np.abs(P - (1.0 - c).reshape(shape))) < 1e-12
+
+
+def test_layered_closed_form(pn):
+    from paper_1908_03301_b200 import inputs
+    rng = np.random.default_rng(5)
+    nx, ny, nz = 12, 7, 9
+    c = rng.uniform(0.2, 2.0, nz).astype(np.float32)
+    e = rng.uniform(0.2, 2.0, nz).astype(np.float32)
+    net = inputs.layered_exact(nx, ny, nz, c, e)
+    _, _, _, flx, _ = gpu_solve(pn, net, 0, 1e-13)
+    assert flx[2] == pytest.approx(ny * float(np.sum(c.astype(np.float64))) / (nx - 1), rel=1e-11)
+    _, _, _, flz, _ = gpu_solve(pn, net, 2, 1e-13)
+    assert flz[2] == pytest.approx(nx * ny / float(np.sum(1.0 / e[:-1].astype(np.float64))), rel=1e-11)
+
+
+def test_worked_example_3x2(pn):
+    """SURVEY.md 8(c) hand-worked example: P(1,0) = 27/71, P(1,1) = 29/71, G_eff = 170/71."""
+    gx = np.array([[[1, 2, 99], [3, 4, 99]]], dtype=np.float32)
+    gy = np.array([[[77, 5, 77], [88, 88, 88]]], dtype=np.float32)
+    h = pn.Network(3, 2, 1)
+    h.set_conductances(gx, gy, None)
+    info = h.solve(0, 1e-13)
+    P = h.pressures().cpu().numpy()
+    fl = h.flux()
+    h.close()
+    assert info.status == pn.PN_OK
+    assert P[0, 0, 1] == pytest.approx(27 / 71, abs=1e-13)
+    assert P[0, 1, 1] == pytest.approx(29 / 71, abs=1e-13)
+    assert fl[0] == pytest.approx(170 / 71, rel=1e-12)
+    assert fl[1] == pytest.approx(170 / 71, rel=1e-12)
+
+
+# ---- degenerate cases -----------------------------------------------------------------------------
+def test_no_spanning_cluster(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(20, 18, 16, seed=3, p=0.08)
+    info, P, fl, ref = compare(pn, oracle, net, 0)
+    assert info.status == pn.PN_NO_SPANNING_CLUSTER and info.inner_iters == 0
+
+
+def test_all_closed(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(8, 8, 8, seed=3, p=0.0)
+    info, P, fl, ref = compare(pn, oracle, net, 2)
+    assert info.n_floating == 8 * 8 * 6
+
+
+def test_series_chain(pn):
+    g = np.array([0.5, 2.0, 0.25, 4.0, 1.0, 9.0], dtype=np.float32)
+    h = pn.Network(6, 1, 1)
+    h.set_conductances(g, np.zeros(6, dtype=np.float32), None)
+    info = h.solve(0, 1e-13)
+    fl = h.flux()
+    h.close()
+    assert fl[2] == pytest.approx(1.0 / float(np.sum(1.0 / g[:5].astype(np.float64))), rel=1e-12)
+
+
+def test_thin_axis(pn, oracle):
+    """Three node planes along the solve axis: every unknown touches both Dirichlet planes."""
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.iid_diluted(3, 21, 10, seed=1, p=0.8), 0)
+    compare(pn, oracle, inputs.iid_diluted(21, 10, 3, seed=1, p=0.8), 2)
+
+
+def test_resolve_and_direction_switch(pn, oracle):
+    """One handle, several solves: directions and networks can change between calls."""
+    from paper_1908_03301_b200 import inputs
+    a = inputs.iid_diluted(18, 14, 11, seed=21, p=0.7)
+    b = inputs.iid_diluted(18, 14, 11, seed=22, p=1.0)
+    h = pn.Network(18, 14, 11)
+    for net, d in ((a, 0), (a, 2), (b, 1), (a, 0)):
+        h.set_conductances(net.gx, net.gy, net.gz)
+        info = h.solve(d, 1e-12)
+        ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, d, 1e-13)
+        assert np.max(np.abs(h.pressures().cpu().numpy() - ref.P)) <= P_TOL
+        assert np.max(np.abs(h.pressures_host() - ref.P)) <= P_TOL
+        assert abs(h.flux()[2] - ref.g_eff) <= G_TOL * abs(ref.g_eff)
+    h.close()
+
+
+def test_device_pointer_inputs(pn, oracle):
+    import torch
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg4_fbm_cut_3d(24, 20, 16)
+    h = pn.Network(net.nx, net.ny, net.nz)
+    h.set_conductances(*(torch.from_numpy(g).cuda() for g in (net.gx, net.gy, net.gz)))
+    h.solve(0, 1e-12)
+    ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, 0, 1e-13)
+    assert np.max(np.abs(h.pressures().cpu().numpy() - ref.P)) <= P_TOL
+    h.close()
+
+
+def test_error_paths(pn):
+    h = pn.Network(8, 6, 4)
+    with pytest.raises(pn.PnError) as e:
+        h.solve(0, 1e-10)
+    assert e.value.code == pn.PN_ERR_STATE
+    g = np.ones((4, 6, 8), dtype=np.float32)
+    bad = g.copy()
+    bad[1, 2, 3] = -1.0
+    with pytest.raises(pn.PnError) as e:
+        h.set_conductances(bad, g, g)
+    assert e.value.code == pn.PN_ERR_VALUE
+    bad[1, 2, 3] = np.nan
+    with pytest.raises(pn.PnError) as e:
+        h.set_conductances(g, bad, g)
+    assert e.value.code == pn.PN_ERR_VALUE
+    # a bad value on an entry that is NOT a bond (forward neighbour off-lattice) is ignored
+    edge = g.copy()
+    edge[:, :, 7] = np.nan
+    h.set_conductances(edge, g, g)
+    with pytest.raises(pn.PnError) as e:
+        h.set_conductances(g, g, None)
+    assert e.value.code == pn.PN_ERR_ARG
+    h.set_conductances(g, g, g)
+    for d, tol in ((3, 1e-10), (-1, 1e-10), (0, 0.0), (0, 2.0)):
+        with pytest.raises(pn.PnError) as e:
+            h.solve(d, tol)
+        assert e.value.code == pn.PN_ERR_ARG
+    with pytest.raises(pn.PnError) as e:
+        h.flux()
+    assert e.value.code == pn.PN_ERR_STATE
+    h.solve(1, 1e-10)
+    h.flux()
+    h.close()
+    h2 = pn.Network(8, 2, 1)
+    h2.set_conductances(np.ones(16, dtype=np.float32), np.ones(16, dtype=np.float32), None)
+    with pytest.raises(pn.PnError) as e:
+        h2.solve(1, 1e-10)          # only 2 node planes along y
+    assert e.value.code == pn.PN_ERR_ARG
+    h2.close()
+
+
+def test_max_iters_status(pn):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg2_fbm_2d(128, 128)
+    info, *_ = gpu_solve(pn, net, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40})
+    assert info.status == pn.PN_MAX_ITERS
+    assert 40 <= info.inner_iters <= 40 + 64
+    assert info.rel_residual > 1e-12
+
+
+def test_deterministic(pn):
+    """Fixed-order grid reductions: two solves of the same input agree bit for bit."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg3_percolation_3d(40, 40, 40)
+    a = gpu_solve(pn, net, 0, 1e-10)
+    b = gpu_solve(pn, net, 0, 1e-10)
+    assert a[0].inner_iters == b[0].inner_iters
+    assert np.array_equal(a[1], b[1])
+    assert a[3] == b[3]
