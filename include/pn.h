@@ -67,6 +67,10 @@ typedef struct {
     long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
     double t_label_ms;     /* S1 + set-up (labelling, pruning, scaling), device time                */
     double t_solve_ms;     /* S3..S7 loop, device time                                              */
+    double t_stencil_ms;   /* with PN_OPT_PROFILE: summed device time of the S4 kernel launches ...  */
+    double t_update_ms;    /* ... and of the S5 kernel launches (CUDA events on the handle's stream) */
+    int n_timed_iters;     /* ... over this many inner iterations                                   */
+    int reserved2;
 } pn_info;
 
 /* options for pn_set_option */
@@ -80,8 +84,10 @@ enum {
     PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32)            */
     PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
-    PN_OPT_KERNEL = 5       /* S4 kernel variant: 0 = default (fastest), 1 = reference kernel that
+    PN_OPT_KERNEL = 5,      /* S4 kernel variant: 0 = default (fastest), 1 = reference kernel that
                                reads neighbours through the caches (kept for cross-checks)          */
+    PN_OPT_PROFILE = 6      /* 1: record CUDA events around every S4 / S5 launch and report the
+                               summed kernel times in pn_info (default 0)                           */
 };
 
 /* Device bytes pn_create needs for an nx x ny x nz lattice (0 on a bad shape). */

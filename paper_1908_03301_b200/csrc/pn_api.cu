@@ -33,7 +33,9 @@ struct pn_ctx {
     bool have_g, have_solution;
     int last_dir_user;
     // options
-    int max_iters, chunk, x0_linear, skip_label, variant;
+    int max_iters, chunk, x0_linear, skip_label, variant, profile;
+    cudaEvent_t* pev;           // event pool for PN_OPT_PROFILE (2*chunk+1), created on demand
+    int pev_n;
     double delta;
     long long launches;
     double flux[4];
@@ -188,6 +190,8 @@ int pn_destroy(pn_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     if (ctx->h_state) cudaFreeHost(ctx->h_state);
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    for (int i = 0; i < ctx->pev_n; ++i) cudaEventDestroy(ctx->pev[i]);
+    delete[] ctx->pev;
     delete ctx;
     return PN_OK;
 }
@@ -201,6 +205,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
         case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
+        case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
 }
@@ -306,6 +311,16 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     int outer = 1;
     int status = PN_OK;
     int total_iters = 0;
+    double t_stencil = 0.0, t_update = 0.0;
+    int n_timed = 0;
+    if (ctx->profile && ctx->pev_n < 2 * ctx->chunk + 1) {
+        for (int i = 0; i < ctx->pev_n; ++i) cudaEventDestroy(ctx->pev[i]);
+        delete[] ctx->pev;
+        ctx->pev_n = 2 * ctx->chunk + 1;
+        ctx->pev = new (std::nothrow) cudaEvent_t[ctx->pev_n];
+        if (!ctx->pev) { ctx->pev_n = 0; return PN_ERR_ARG; }
+        for (int i = 0; i < ctx->pev_n; ++i) CK(cudaEventCreate(&ctx->pev[i]));
+    }
 
     if (n_solved == 0 || !(nb > 0.0)) {
         status = PN_NO_SPANNING_CLUSTER;
@@ -321,10 +336,21 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         CK(pn_launch_set_state(P, rr_hat, 0.0, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 1, s, &nl));
         double best_rn = rn;
         int stagnant = 0;
+        int iters_seen = 0;
         while (true) {
-            CK(pn_launch_inner(g, P, ctx->chunk, ctx->variant, s, &nl));
+            CK(pn_launch_inner(g, P, ctx->chunk, ctx->variant, s, &nl, ctx->profile ? ctx->pev : nullptr));
             rc = read_state(ctx);
             if (rc) return rc;
+            if (ctx->profile) {   // per-kernel device time of the launches that did work (not the no-op tail)
+                const int ran = h->iters - iters_seen;
+                for (int it = 0; it < ran && it < ctx->chunk; ++it) {
+                    float ta = 0.f, tb = 0.f;
+                    cudaEventElapsedTime(&ta, ctx->pev[2 * it], ctx->pev[2 * it + 1]);
+                    cudaEventElapsedTime(&tb, ctx->pev[2 * it + 1], ctx->pev[2 * it + 2]);
+                    t_stencil += ta; t_update += tb; ++n_timed;
+                }
+            }
+            iters_seen = h->iters;
             if (h->flag == PN_FLAG_RUN) continue;
             total_iters = h->iters;
             if (h->flag == PN_FLAG_BREAKDOWN) { status = PN_ERR_BREAKDOWN; }
@@ -367,6 +393,9 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         info->n_floating = (long long)h->count[3];
         if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
         if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
+        info->t_stencil_ms = t_stencil;
+        info->t_update_ms = t_update;
+        info->n_timed_iters = n_timed;
     }
     return status;
 }

@@ -150,13 +150,17 @@ int grid_for(long long work_items) {
 }  // namespace
 
 cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int variant, cudaStream_t st,
-                            int* launches) {
+                            int* launches, cudaEvent_t* ev) {
     const int nvec = (int)(g.npad / 4);
     const int nb = grid_for(nvec);
     (void)variant;
+    // ev (optional, 2*iterations+1 events): kernel boundaries, for the per-kernel timing of PN_OPT_PROFILE
+    if (ev) cudaEventRecord(ev[0], st);
     for (int it = 0; it < iterations; ++it) {
         k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2);
+        if (ev) cudaEventRecord(ev[2 * it + 1], st);
         k_update<<<nb, TPB, 0, st>>>(nvec, P);
+        if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
     *launches += 2 * iterations;
     return cudaGetLastError();
