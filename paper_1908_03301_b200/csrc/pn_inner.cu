@@ -149,19 +149,29 @@ int grid_for(long long work_items) {
 
 }  // namespace
 
+// variant: 0 = automatic (TMA kernel on lattices large enough to fill the GPU, reference kernel below that),
+//          1 = reference kernel, 2 = TMA kernel whatever the size.
 cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int variant, cudaStream_t st,
                             int* launches, cudaEvent_t* ev) {
     const int nvec = (int)(g.npad / 4);
     const int nb = grid_for(nvec);
-    (void)variant;
+    bool use_tma = variant == 2 || (variant == 0 && g.npad >= (1ll << 21));
+    pn_tma_plan* plan = nullptr;
+    if (use_tma && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) {
+        if (variant == 2) return cudaErrorNotSupported;   // asked for explicitly: fail loudly
+        use_tma = false;
+    }
     // ev (optional, 2*iterations+1 events): kernel boundaries, for the per-kernel timing of PN_OPT_PROFILE
+    cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);
-    for (int it = 0; it < iterations; ++it) {
-        k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2);
+    for (int it = 0; it < iterations && e == cudaSuccess; ++it) {
+        if (use_tma) e = pn_launch_stencil_tma(plan, g, P, st);
+        else k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2);
         if (ev) cudaEventRecord(ev[2 * it + 1], st);
         k_update<<<nb, TPB, 0, st>>>(nvec, P);
         if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
+    pn_tma_plan_free(plan);
     *launches += 2 * iterations;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -135,3 +135,10 @@ cudaError_t pn_launch_flux(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, 
 cudaError_t pn_launch_export_x(const pn_geom& g, const pn_ptrs& P, double* out, cudaStream_t st, int* launches);
 cudaError_t pn_launch_export_cls(const pn_geom& g, const pn_ptrs& P, signed char* out, int user_dir_is_2d,
                                  cudaStream_t st, int* launches);
+
+// TMA-fed S4 kernel (pn_stencil_tma.cu)
+struct pn_tma_plan;
+bool pn_tma_supported();
+bool pn_tma_plan_build(pn_tma_plan** out, const pn_geom& g, const pn_ptrs& P);
+void pn_tma_plan_free(pn_tma_plan* pl);
+cudaError_t pn_launch_stencil_tma(const pn_tma_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);

@@ -102,6 +102,7 @@ def test_cfg5_sibling(pn, oracle, direction):
 
 
 def test_cfg4_sibling_128(pn, oracle):
+    """2^21 nodes: the size from which the automatic choice is the TMA kernel."""
     from paper_1908_03301_b200 import inputs
     compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13)
 
@@ -110,26 +111,47 @@ def test_cfg4_sibling_128(pn, oracle):
 @pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 31, 7), (130, 6, 3)])
 @pytest.mark.parametrize("direction", [0, 1, 2])
 @pytest.mark.parametrize("p", [1.0, 0.6])
-def test_ragged_3d(pn, oracle, shape, direction, p):
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
+    """kernel 1 = reference S4 kernel, 2 = TMA-fed 2.5D kernel (forced, whatever the size)."""
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(*shape, seed=7 + direction, p=p)
-    compare(pn, oracle, net, direction)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
 @pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (3, 64), (257, 31)])
 @pytest.mark.parametrize("direction", [0, 1])
 @pytest.mark.parametrize("p", [1.0, 0.7])
-def test_ragged_2d(pn, oracle, shape, direction, p):
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(shape[0], shape[1], 1, seed=11 + direction, p=p)
-    compare(pn, oracle, net, direction)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-def test_reference_kernel_variant(pn, oracle):
-    """The reference stencil kernel (PN_OPT_KERNEL = 1) must pass the same parity bar."""
+@pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
+def test_tma_kernel_multi_tile(pn, oracle, shape, direction):
+    """Lattices wider than one 256-node TMA box and taller than one 8-row tile: x and y halos between
+    tiles, several z chunks, ragged tails in all three directions."""
     from paper_1908_03301_b200 import inputs
-    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(40, 36, 33), 0, opts={pn.PN_OPT_KERNEL: 1})
-    compare(pn, oracle, inputs.cfg1_iid_2d(), 0, opts={pn.PN_OPT_KERNEL: 1})
+    net = inputs.iid_diluted(*shape, seed=5, p=0.75)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 2})
+
+
+def test_tma_kernel_2d_wide(pn, oracle):
+    """2D lattice wider than the 2048-node tile of the 2D configuration (x halo between tiles)."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(2100, 40, 1, seed=9, p=1.0)
+    compare(pn, oracle, net, 1, opts={pn.PN_OPT_KERNEL: 2})
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_kernel_variants(pn, oracle, kernel):
+    """Both S4 kernels must pass the same parity bar (0 = automatic choice is what the other tests use)."""
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(40, 36, 33), 0, opts={pn.PN_OPT_KERNEL: kernel})
+    compare(pn, oracle, inputs.cfg1_iid_2d(), 0, opts={pn.PN_OPT_KERNEL: kernel})
+    compare(pn, oracle, inputs.cfg3_percolation_3d(64, 64, 64), 0, opts={pn.PN_OPT_KERNEL: kernel})
 
 
 def test_zero_start_and_restart_options(pn, oracle):
