@@ -70,7 +70,8 @@ def _load():
                                                         ctypes.POINTER(ctypes.c_byte),
                                                         ctypes.POINTER(_Info)]
         _lib.pno_solve.restype = ctypes.c_int
-        _lib.pno_certificate.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, dp, dp, dp]
+        _lib.pno_certificate.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, dp, dp, dp,
+                                         ctypes.POINTER(ctypes.c_byte)]
         _lib.pno_certificate.restype = ctypes.c_int
     return _lib
 
@@ -107,7 +108,9 @@ def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, threa
                          info.t_label, info.t_assemble, info.t_pcg, info.nnz)
 
 
-def certificate(nx, ny, nz, gx, gy, gz, P, direction=0):
+def certificate(nx, ny, nz, gx, gy, gz, P, direction=0, classes_out=None):
+    """(rel_residual, pin_err) of any pressure field; `classes_out` (int8 array of N entries, optional)
+    receives the node classes of the serial labelling."""
     lib = _load()
     gx, gy, gz = (_prep(nx, ny, nz, g) for g in (gx, gy, gz))
     P = np.ascontiguousarray(P, dtype=np.float64)
@@ -115,7 +118,7 @@ def certificate(nx, ny, nz, gx, gy, gz, P, direction=0):
     pin = ctypes.c_double()
     rc = lib.pno_certificate(nx, ny, nz, _ptr(gx, ctypes.c_float), _ptr(gy, ctypes.c_float),
                              _ptr(gz, ctypes.c_float), direction, _ptr(P, ctypes.c_double),
-                             ctypes.byref(rel), ctypes.byref(pin))
+                             ctypes.byref(rel), ctypes.byref(pin), _ptr(classes_out, ctypes.c_byte))
     if rc < 0:
         raise ValueError(f"pno_certificate failed with code {rc}")
     return rel.value, pin.value

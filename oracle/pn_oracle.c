@@ -348,15 +348,16 @@ int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const fl
 }
 
 /* Independent residual certificate of ANY pressure field (S8c last pin row): ||b - A P_S||2/||b||2 with
- * this file's assembled operator, and max |P - pin| over Dirichlet and pinned nodes. */
+ * this file's assembled operator, and max |P - pin| over Dirichlet and pinned nodes.  classes_out (N bytes,
+ * may be NULL) receives the node classes of the serial labelling. */
 int pno_certificate(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction,
-                    const double *P, double *rel_residual, double *pin_err) {
+                    const double *P, double *rel_residual, double *pin_err, signed char *classes_out) {
     lattice L;
     pno_info info;
     memset(&info, 0, sizeof(info));
     int rc = setup(&L, nx, ny, nz, gx, gy, gz, direction);
     if (rc) return rc;
-    signed char *cls = (signed char *)malloc((size_t)L.N);
+    signed char *cls = classes_out ? classes_out : (signed char *)malloc((size_t)L.N);
     if (!cls || classify(&L, cls, &info)) return -3;
     double pe = 0.0;
     for (long long n = 0; n < L.N; ++n) {
@@ -378,6 +379,6 @@ int pno_certificate(int nx, int ny, int nz, const float *gx, const float *gy, co
         free(x);
         csr_free(&A);
     }
-    free(cls);
+    if (!classes_out) free(cls);
     return 0;
 }
