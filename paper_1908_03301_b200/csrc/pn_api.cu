@@ -51,7 +51,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct layout {
     pn_geom g;
-    size_t off_raw[3], off_gs[3], off_w[3], off_s, off_x64, off_r, off_p, off_p2, off_q, off_xh, off_cls, off_slots,
+    size_t off_raw[3], off_gs[3], off_w[3], off_s, off_x64, off_r, off_p, off_p2, off_q, off_xh, off_r2, off_q2, off_cls, off_slots,
         off_state, total;
     size_t halo;                // elements in one halo plane
 };
@@ -83,6 +83,8 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     L->off_p2 = take(vec * 4);
     L->off_q = take(vec * 4);
     L->off_xh = take(vec * 4);
+    L->off_r2 = take(vec * 4);
+    L->off_q2 = take(vec * 4);
     L->off_cls = take(vec);
     L->off_slots = take(4 * PN_MAX_BLOCKS * sizeof(double));
     L->off_state = take(sizeof(pn_state));
@@ -163,6 +165,8 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     P.p2 = (float*)(ctx->ws + L.off_p2) + h;
     P.q = (float*)(ctx->ws + L.off_q) + h;
     P.xh = (float*)(ctx->ws + L.off_xh) + h;
+    P.r2 = (float*)(ctx->ws + L.off_r2) + h;
+    P.q2 = (float*)(ctx->ws + L.off_q2) + h;
     P.cls = (signed char*)(ctx->ws + L.off_cls) + h;
     P.parent = (int*)P.q;
     P.flags = (int*)P.xh;
@@ -289,17 +293,21 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     CK(cudaEventRecord(ctx->ev[0], s));
     CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + sizeof(P.st->count), s));
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
+    CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
+    const int scheme = pn_resolve_variant(g, ctx->variant);
+    const int fused = scheme == 3;
     const bool do_label = !ctx->skip_label && ctx->h_state->any_closed;
     CK(pn_launch_label(g, P, do_label, ctx->x0_linear, s, &nl));
     // parent / flags aliased q / x_hat: clear the CG vectors before the first iteration
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
     CK(cudaMemsetAsync(P.q, 0, vbytes, s));
+    if (fused) CK(cudaMemsetAsync(P.q2, 0, vbytes, s));
     // p / p2 double as export staging (pn_get_pressures), halo planes included: clear them whole
     const size_t vhalo = ((size_t)g.npad + 2 * (size_t)g.plane) * 4;
     CK(cudaMemsetAsync(P.p - g.plane, 0, vhalo, s));
     CK(cudaMemsetAsync(P.p2 - g.plane, 0, vhalo, s));
-    CK(pn_launch_residual64(g, P, s, &nl));
+    CK(pn_launch_residual64(g, P, fused, s, &nl));
     CK(cudaEventRecord(ctx->ev[1], s));
     rc = read_state(ctx);
     if (rc) return rc;
@@ -338,7 +346,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         int stagnant = 0;
         int iters_seen = 0;
         while (true) {
-            CK(pn_launch_inner(g, P, ctx->chunk, ctx->variant, s, &nl, ctx->profile ? ctx->pev : nullptr));
+            CK(pn_launch_inner(g, P, ctx->chunk, scheme, s, &nl, ctx->profile ? ctx->pev : nullptr));
             rc = read_state(ctx);
             if (rc) return rc;
             if (ctx->profile) {   // per-kernel device time of the launches that did work (not the no-op tail)
@@ -355,10 +363,12 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
             total_iters = h->iters;
             if (h->flag == PN_FLAG_BREAKDOWN) { status = PN_ERR_BREAKDOWN; }
             // S7 + S3: fold the fp32 correction into x64 and recompute the true residual
-            const double rr_before = h->rr_old;   // rr entering the last iteration: beta's denominator
+            // beta's denominator = r.r of the residual that generated the last search direction: the two-kernel
+            // iteration has already stepped past it (rr_old), the fused kernel holds it as its measured rr
+            const double rr_before = fused ? h->rr : h->rr_old;
             const int flag = h->flag;
             CK(pn_launch_flush(g, P, s, &nl));
-            CK(pn_launch_residual64(g, P, s, &nl));
+            CK(pn_launch_residual64(g, P, fused, s, &nl));
             rc = read_state(ctx);
             if (rc) return rc;
             ++outer;

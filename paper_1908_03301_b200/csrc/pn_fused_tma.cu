@@ -1,0 +1,365 @@
+// pn_fused_tma.cu -- the whole fp32 inner CG iteration (SURVEY.md 8(a) S4 + S5 + S6) as ONE 2.5D, TMA-fed,
+// warp-specialised persistent kernel for sm_100a: 44 B per node-iteration instead of the 48 B of the
+// two-kernel form (SURVEY.md 8(d) "irreducible: g once + each of x, r, p, q read once and written once").
+//
+// Paper: K2 (SpMV + dot) and K3 (vector updates + dots) are two kernels because the update of
+// the residual needs alpha = r.r / p.Ap, a grid-wide sum over the SpMV's output.  Here the
+// residual update of iteration t-1 is deferred into the kernel of iteration t, where it is recomputed on
+// the tile halo as well, so that one kernel per iteration remains:
+//
+//   kernel F(t):   r_t = r_{t-1} - alpha_{t-1} q_{t-1}          (tile + one-node halo, from r, q staged by TMA)
+//                  p_t = r_t + beta_t p_{t-1}                   (tile + halo)  -> shared-memory plane ring
+//                  x_hat += alpha_{t-1} p_{t-1}
+//                  q_t = p_t - W p_t                            (7-point operator from the plane ring)
+//                  sums:  rr = r_t.r_t   pq = p_t.q_t   rq = r_t.q_t   qq = q_t.q_t
+//   last block:    alpha_t = rr / pq
+//                  beta_{t+1} = ||r_t - alpha_t q_t||^2 / rr = (rr - 2 alpha_t rq + alpha_t^2 qq) / rr
+//
+// beta_{t+1} must be known before r_{t+1} exists; it is obtained from the three sums by expanding the
+// square (exact in exact arithmetic; in fp32 the fp64-accumulated sums reproduce ||r_{t+1}||^2 to ~1e-7
+// relative unless r shrinks by orders of magnitude in one step, and the NEXT kernel measures the true
+// r_{t+1}.r_{t+1} anyway: alpha_{t+1} and the denominator of beta_{t+2} use the measured value).  A
+// non-positive prediction raises the reliable-update flag, i.e. an fp64 residual replacement.
+// r, p and q are double-buffered (index = iteration parity): a tile reads its neighbours' old values as halo.
+//
+// HBM bytes per node: reads r, q, p, x_hat, wx, wy, wz (28 B) + writes r, q, p, x_hat (16 B) = 44 B.
+#include <new>
+
+#include "pn_tma.cuh"
+
+namespace {
+
+using namespace pn_tma;
+
+template <int NBX_, int TY_, bool HAS_Y_, int S_>
+struct FCfg {
+    static constexpr int NBX = NBX_, TY = TY_, S = S_;
+    static constexpr bool HAS_Y = HAS_Y_;
+    static constexpr int BOXW = 256;                       // TMA box limit per dimension
+    static constexpr int TXW = BOXW * NBX;                 // tile width in nodes
+    static constexpr int RH = TY + (HAS_Y ? 2 : 0);        // rows of r, q, p and p_new including the y halo
+    static constexpr int RWY = TY + (HAS_Y ? 1 : 0);       // rows of the wy box (backward row included)
+    static constexpr int W = TXW + 8;                      // p_new ring row: 4 pad + tile + 4 pad floats
+    static constexpr int NCONS = 64 * NBX * TY;            // consumer threads: one float4 of nodes each
+    static constexpr int NTHREADS = NCONS + 32;            // + one producer warp
+    static constexpr int NHALO4 = HAS_Y ? 2 * 64 * NBX : 0;  // float4s in the two halo rows
+    // stage layout (floats): three haloed vectors, then the weights
+    static constexpr int VEC = NBX * RH * BOXW + 2 * a32(RH * 4);   // main boxes, left sliver, right sliver
+    static constexpr int V_SL = NBX * RH * BOXW;
+    static constexpr int V_SR = V_SL + a32(RH * 4);
+    static constexpr int R_ = 0, Q_ = VEC, P_ = 2 * VEC;
+    static constexpr int WX = 3 * VEC;
+    static constexpr int WX_SL = WX + NBX * TY * BOXW;
+    static constexpr int WY = WX_SL + a32(TY * 4);
+    static constexpr int WZ = WY + (HAS_Y ? NBX * RWY * BOXW : 0);
+    static constexpr int STAGE_FLOATS = WZ + NBX * TY * BOXW;
+    static constexpr int RING_FLOATS = 4 * RH * W;
+    static constexpr size_t SMEM_BYTES = (size_t)(S * STAGE_FLOATS + RING_FLOATS) * 4 + 2 * S * 8 + 64 * 8 + 1024;
+    // transaction bytes per group of boxes
+    static constexpr unsigned B_RQP = 3u * (NBX * RH * BOXW + 2 * RH * 4) * 4u;
+    static constexpr unsigned B_W = (NBX * TY * BOXW + TY * 4 + (HAS_Y ? NBX * RWY * BOXW : 0)) * 4u;
+    static constexpr unsigned B_WZ = NBX * TY * BOXW * 4u;
+};
+
+struct alignas(64) pn_fmaps {
+    CUtensorMap v_main[3][2], v_slv[3][2];   // [r, q, p][buffer]
+    CUtensorMap wx_main, wx_slv, wy, wz;
+};
+
+// Last-block epilogue: alpha_t, the predicted beta_{t+1}, bookkeeping and the triggers the host polls for.
+__device__ __forceinline__ void finish_F(pn_state* st, double rr, double pq, double rq, double qq) {
+    st->rr_old = st->rr;
+    st->rr = rr;
+    st->pq = pq;
+    const int it = st->iters + 1;
+    st->iters = it;
+    double rr_max = st->rr_max;
+    if (rr > rr_max) { rr_max = rr; st->rr_max = rr_max; }
+    int flag = PN_FLAG_RUN;
+    double alpha = 0.0, beta = 0.0;
+    if (!(rr >= 0.0) || isinf(rr)) flag = PN_FLAG_BREAKDOWN;
+    else if (rr == 0.0) flag = PN_FLAG_CONVERGED;
+    else if (!(pq > 0.0) || isinf(pq)) flag = PN_FLAG_BREAKDOWN;
+    else {
+        alpha = rr / pq;
+        const double rr_next = rr - 2.0 * alpha * rq + alpha * alpha * qq;   // ||r_t - alpha_t q_t||^2
+        if (rr <= st->rr_target) flag = PN_FLAG_CONVERGED;
+        else if (rr < st->delta2 * rr_max) flag = PN_FLAG_UPDATE;
+        else if (it >= st->max_iters) flag = PN_FLAG_BUDGET;
+        else if (!(rr_next > 0.0) || isinf(rr_next)) flag = PN_FLAG_UPDATE;   // prediction lost: replace the residual
+        else beta = rr_next / rr;
+    }
+    st->alpha = alpha;      // alpha_t: next kernel's residual and solution updates
+    st->alpha_x = alpha;    // ... and what k_flush applies to the pending direction p_t
+    st->beta = beta;
+    st->flag = flag;
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NTHREADS, 1)
+k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    float* stages = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    float* ring = stages + C::S * C::STAGE_FLOATS;
+    uint64_t* full = reinterpret_cast<uint64_t*>(ring + C::RING_FLOATS);
+    uint64_t* empty = full + C::S;
+    double* red = reinterpret_cast<double*>(empty + C::S);   // 32 doubles + 4 totals
+
+    const int tid = threadIdx.x;
+    const float beta = (float)st->beta;
+    const float al = (float)st->alpha;          // alpha_{t-1} (0 right after a residual replacement)
+    const float nal = -al;
+    const int par = st->iters & 1;              // buffers holding r_{t-1}, q_{t-1}, p_{t-1}
+    float* __restrict__ r_out = par ? P.r : P.r2;
+    float* __restrict__ q_out = par ? P.q : P.q2;
+    float* __restrict__ p_out = par ? P.p : P.p2;
+
+    if (tid == 0) {
+        for (int s = 0; s < C::S; ++s) {
+            mbar_init(full + s, 1);
+            mbar_init(empty + s, C::NCONS / 32);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int tiles = ntx * nty;
+    const int total = tiles * nchunks;
+    double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
+
+    if (tid >= C::NCONS) {
+        // ================= producer warp: one elected lane issues every TMA load =================
+        if (tid == C::NCONS) {
+            unsigned it = 0;
+            for (int item = blockIdx.x; item < total; item += gridDim.x) {
+                const int chunk = item / tiles, t = item - chunk * tiles;
+                const int tyi = t / ntx, txi = t - tyi * ntx;
+                const int x0 = txi * C::TXW, y0 = tyi * C::TY, k0 = chunk * lz;
+                const int k1 = min(k0 + lz, g.nz);
+                const int yh = y0 - (C::HAS_Y ? 1 : 0);
+                for (int kk = k0 - 2; kk < k1; ++kk, ++it) {
+                    const int s = it % C::S;
+                    const unsigned ph = (it / C::S) & 1u;
+                    mbar_wait(empty + s, ph ^ 1u);
+                    float* sg = stages + s * C::STAGE_FLOATS;
+                    const bool has_w = kk >= k0;
+                    const bool has_wz = kk >= k0 - 1;
+                    mbar_expect_tx(full + s, C::B_RQP + (has_w ? C::B_W : 0u) + (has_wz ? C::B_WZ : 0u));
+                    const int zp = kk + 2;   // plane kk+1 (+1: the tensor maps start at the leading halo plane)
+                    const int zw = kk + 1;   // plane kk
+#pragma unroll
+                    for (int v = 0; v < 3; ++v) {
+                        float* sv = sg + v * C::VEC;
+#pragma unroll
+                        for (int b = 0; b < C::NBX; ++b)
+                            tma_load_3d(sv + b * C::RH * C::BOXW, &maps.v_main[v][par], x0 + b * C::BOXW, yh, zp, full + s);
+                        tma_load_3d(sv + C::V_SL, &maps.v_slv[v][par], x0 - 4, yh, zp, full + s);
+                        tma_load_3d(sv + C::V_SR, &maps.v_slv[v][par], x0 + C::TXW, yh, zp, full + s);
+                    }
+                    if (has_w) {
+#pragma unroll
+                        for (int b = 0; b < C::NBX; ++b) {
+                            tma_load_3d(sg + C::WX + b * C::TY * C::BOXW, &maps.wx_main, x0 + b * C::BOXW, y0, zw, full + s);
+                            if (C::HAS_Y)
+                                tma_load_3d(sg + C::WY + b * C::RWY * C::BOXW, &maps.wy, x0 + b * C::BOXW, yh, zw, full + s);
+                        }
+                        tma_load_3d(sg + C::WX_SL, &maps.wx_slv, x0 - 4, y0, zw, full + s);
+                    }
+                    if (has_wz) {
+#pragma unroll
+                        for (int b = 0; b < C::NBX; ++b)
+                            tma_load_3d(sg + C::WZ + b * C::TY * C::BOXW, &maps.wz, x0 + b * C::BOXW, y0, zw, full + s);
+                    }
+                }
+            }
+        }
+    } else {
+        // ================= consumer warps ==========================================================
+        const int lane = tid & 31;
+        const int tx = tid % (64 * C::NBX), ty = tid / (64 * C::NBX);
+        const int b = tx >> 6, c4 = tx & 63;
+        const int rrow = ty + (C::HAS_Y ? 1 : 0);               // own row in the haloed arrays
+        const int rcol = 4 + b * C::BOXW + c4 * 4;              // own column in a ring row
+        const int own_main = (b * C::RH + rrow) * C::BOXW + c4 * 4;   // own float4 inside the r / q / p main boxes
+        const int own_ty = (b * C::TY + ty) * C::BOXW + c4 * 4;       // own float4 inside the wx / wz boxes
+        // the float4 of the two halo rows this thread also owns in phase A (the LAST warps take them)
+        const int hidx = tid - (C::NCONS - C::NHALO4);
+        const bool has_halo = C::HAS_Y && hidx >= 0;
+        const int hb = has_halo ? hidx / 128 : 0;
+        const int hrow = has_halo ? (((hidx >> 6) & 1) ? C::RH - 1 : 0) : 0;
+        const int hc4 = hidx & 63;
+        unsigned it = 0;
+        for (int item = blockIdx.x; item < total; item += gridDim.x) {
+            const int chunk = item / tiles, t = item - chunk * tiles;
+            const int tyi = t / ntx, txi = t - tyi * ntx;
+            const int x0 = txi * C::TXW, y0 = tyi * C::TY, k0 = chunk * lz;
+            const int k1 = min(k0 + lz, g.nz);
+            const int x = x0 + b * C::BOXW + c4 * 4, y = y0 + ty;
+            const bool inb = (x < g.px) && (y < g.ny);
+            const long long nrow = (long long)y * g.px + x;
+            float4 wzm = make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 r_cur = make_float4(0.f, 0.f, 0.f, 0.f);     // r_t on the own float4 of plane kk
+            float4 xh_nxt = make_float4(0.f, 0.f, 0.f, 0.f);    // x_hat of plane kk+1, fetched one step ahead
+            if (inb) xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)k0 * g.plane + nrow);
+            bar_consumers(C::NCONS);   // the ring is rebuilt per item: nobody may still read the previous item's planes
+            for (int kk = k0 - 2; kk < k1; ++kk, ++it) {
+                const int s = it % C::S;
+                const unsigned ph = (it / C::S) & 1u;
+                // x_hat of plane kk+2 goes in flight now and is used one step later
+                const float4 xh_use = xh_nxt;
+                if (inb && kk + 2 >= k0 + 1 && kk + 2 < k1)
+                    xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)(kk + 2) * g.plane + nrow);
+                mbar_wait(full + s, ph);
+                const float* sg = stages + s * C::STAGE_FLOATS;
+                // ---- phase A: r_t, p_t on plane kk+1 (tile and halo) -> ring; own part -> HBM ----
+                float* rw = ring + ((kk + 5) & 3) * (C::RH * C::W);
+                float4 r_nxt;
+                {
+                    const float4 po = lds4(sg + C::P_ + own_main);
+                    r_nxt = fma4(nal, lds4(sg + C::Q_ + own_main), lds4(sg + C::R_ + own_main));
+                    const float4 pn = fma4(beta, po, r_nxt);
+                    *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
+                    if (kk + 1 >= k0 && kk + 1 < k1 && inb) {
+                        const long long n = (long long)(kk + 1) * g.plane + nrow;
+                        *reinterpret_cast<float4*>(r_out + n) = r_nxt;
+                        *reinterpret_cast<float4*>(p_out + n) = pn;
+                        *reinterpret_cast<float4*>(P.xh + n) = fma4(al, po, xh_use);
+                        a_rr += (double)dot4(r_nxt, r_nxt);
+                    }
+                }
+                if (has_halo) {
+                    const int o = (hb * C::RH + hrow) * C::BOXW + hc4 * 4;
+                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
+                    *reinterpret_cast<float4*>(rw + hrow * C::W + 4 + hb * C::BOXW + hc4 * 4) = fma4(beta, lds4(sg + C::P_ + o), rn);
+                }
+                if (tid < 2 * C::RH) {
+                    const int side = tid / C::RH, row = tid - side * C::RH;
+                    const int o = (side ? C::V_SR : C::V_SL) + row * 4;
+                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
+                    *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + C::TXW : 0)) = fma4(beta, lds4(sg + C::P_ + o), rn);
+                }
+                bar_consumers(C::NCONS);
+                // ---- phase C: q_t(kk) = p_t - W p_t from the ring, weights from the stage ----
+                if (kk >= k0) {
+                    const float* r0 = ring + ((kk + 4) & 3) * (C::RH * C::W) + rrow * C::W + rcol;
+                    const float4 pc = lds4(r0);
+                    const float4 pzm = lds4(ring + ((kk + 3) & 3) * (C::RH * C::W) + rrow * C::W + rcol);
+                    const float4 pzp = lds4(rw + rrow * C::W + rcol);
+                    float pl = __shfl_up_sync(0xffffffffu, pc.w, 1);
+                    float pr = __shfl_down_sync(0xffffffffu, pc.x, 1);
+                    if (lane == 0) pl = r0[-1];
+                    if (lane == 31) pr = r0[4];
+                    const float4 gx = lds4(sg + C::WX + own_ty);
+                    float gxl = __shfl_up_sync(0xffffffffu, gx.w, 1);
+                    if (lane == 0) {
+                        if (c4 != 0) gxl = sg[C::WX + own_ty - 1];
+                        else if (b != 0) gxl = sg[C::WX + ((b - 1) * C::TY + ty) * C::BOXW + C::BOXW - 1];
+                        else gxl = sg[C::WX_SL + ty * 4 + 3];
+                    }
+                    const float4 gz = lds4(sg + C::WZ + own_ty);
+                    float4 q;
+                    q.x = gxl * pl + gx.x * pc.y + wzm.x * pzm.x + gz.x * pzp.x;
+                    q.y = gx.x * pc.x + gx.y * pc.z + wzm.y * pzm.y + gz.y * pzp.y;
+                    q.z = gx.y * pc.y + gx.z * pc.w + wzm.z * pzm.z + gz.z * pzp.z;
+                    q.w = gx.z * pc.z + gx.w * pr + wzm.w * pzm.w + gz.w * pzp.w;
+                    if (C::HAS_Y) {
+                        const float4 pym = lds4(r0 - C::W), pyp = lds4(r0 + C::W);
+                        const int oy = (b * C::RWY + ty) * C::BOXW + c4 * 4;   // row ty of the wy box = lattice row y-1
+                        const float4 gym = lds4(sg + C::WY + oy), gy = lds4(sg + C::WY + oy + C::BOXW);
+                        q.x += gym.x * pym.x + gy.x * pyp.x;
+                        q.y += gym.y * pym.y + gy.y * pyp.y;
+                        q.z += gym.z * pym.z + gy.z * pyp.z;
+                        q.w += gym.w * pym.w + gy.w * pyp.w;
+                    }
+                    q.x = pc.x - q.x; q.y = pc.y - q.y; q.z = pc.z - q.z; q.w = pc.w - q.w;
+                    if (inb) {
+                        *reinterpret_cast<float4*>(q_out + (long long)kk * g.plane + nrow) = q;
+                        a_pq += (double)dot4(pc, q);
+                        a_rq += (double)dot4(r_cur, q);
+                        a_qq += (double)dot4(q, q);
+                    }
+                    wzm = gz;
+                } else if (kk == k0 - 1) {
+                    wzm = lds4(sg + C::WZ + own_ty);   // wz(k0-1): the backward z bond of the first plane
+                }
+                r_cur = r_nxt;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + s);
+            }
+        }
+    }
+    // ---- the four sums: warp -> block -> grid; the last block computes alpha_t and beta_{t+1} ----
+    a_rr = pn_block_sum(a_rr, red);
+    a_pq = pn_block_sum(a_pq, red);
+    a_rq = pn_block_sum(a_rq, red);
+    a_qq = pn_block_sum(a_qq, red);
+    const double v4[4] = {a_rr, a_pq, a_rq, a_qq};
+    if (pn_grid_sum<4>(v4, P.slots, &st->ticket, red, red + 32)) {
+        if (threadIdx.x == 0) finish_F(st, red[32], red[33], red[34], red[35]);
+    }
+}
+
+// ---- host side ----------------------------------------------------------------------------------------
+template <class C>
+bool build_maps(pn_fmaps* M, const pn_geom& g, const pn_ptrs& P) {
+    const long long h = g.plane;
+    const float* vec[3][2] = {{P.r, P.r2}, {P.q, P.q2}, {P.p, P.p2}};
+    bool ok = true;
+    for (int v = 0; v < 3; ++v)
+        for (int bsel = 0; bsel < 2; ++bsel) {
+            ok &= make_map(&M->v_main[v][bsel], g, vec[v][bsel] - h, C::BOXW, C::RH);
+            ok &= make_map(&M->v_slv[v][bsel], g, vec[v][bsel] - h, 4, C::RH);
+        }
+    ok &= make_map(&M->wx_main, g, P.w[0] - h, C::BOXW, C::TY);
+    ok &= make_map(&M->wx_slv, g, P.w[0] - h, 4, C::TY);
+    ok &= make_map(&M->wy, g, P.w[1] - h, C::BOXW, C::RWY);
+    ok &= make_map(&M->wz, g, P.w[2] - h, C::BOXW, C::TY);
+    return ok;
+}
+
+template <class C>
+cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int ntx = (g.px + C::TXW - 1) / C::TXW, nty = (g.ny + C::TY - 1) / C::TY;
+    const int sms = pn_sm_count();
+    const int lz = choose_lz(g.nz, ntx * nty, sms, 44.0, 24.0);   // two extra planes of r, q, p per chunk
+    const int nchunks = (g.nz + lz - 1) / lz;
+    const long long total = (long long)ntx * nty * nchunks;
+    const int nb = (int)(total < sms ? total : sms);
+    k_cg_fused_tma<C><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(M, g, P, ntx, nty, nchunks, lz);
+    return cudaGetLastError();
+}
+
+typedef FCfg<1, 8, true, 3> FCfg3D;    // 256 x 8 tile, y halo, 3 stages
+typedef FCfg<8, 1, false, 4> FCfg2D;   // 2048 x 1 tile (lattices held as nx x 1 x ny), 4 stages
+
+}  // namespace
+
+struct pn_fused_plan {
+    pn_fmaps maps;
+    bool is2d;
+};
+
+bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P) {
+    if (!get_encoder()) return false;
+    pn_fused_plan* pl = new (std::nothrow) pn_fused_plan;
+    if (!pl) return false;
+    pl->is2d = (g.ny == 1);
+    const bool ok = pl->is2d ? build_maps<FCfg2D>(&pl->maps, g, P) : build_maps<FCfg3D>(&pl->maps, g, P);
+    if (!ok) { delete pl; return false; }
+    *out = pl;
+    return true;
+}
+
+void pn_fused_plan_free(pn_fused_plan* pl) { delete pl; }
+
+cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st) {
+    return pl->is2d ? launch_cfg<FCfg2D>(g, P, pl->maps, st) : launch_cfg<FCfg3D>(g, P, pl->maps, st);
+}

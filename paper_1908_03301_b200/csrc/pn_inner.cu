@@ -149,29 +149,36 @@ int grid_for(long long work_items) {
 
 }  // namespace
 
-// variant: 0 = automatic (TMA kernel on lattices large enough to fill the GPU, reference kernel below that),
-//          1 = reference kernel, 2 = TMA kernel whatever the size.
-cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int variant, cudaStream_t st,
+// PN_OPT_KERNEL: 0 = automatic (single fused TMA kernel on lattices large enough to fill the GPU, reference
+// kernels below that), 1 = reference two-kernel iteration, 2 = two-kernel iteration with the TMA S4 kernel,
+// 3 = single fused TMA kernel whatever the size.
+int pn_resolve_variant(const pn_geom& g, int variant) {
+    if (variant == 0) return (g.npad >= (1ll << 21) && pn_tma_supported()) ? 3 : 1;
+    return variant;
+}
+
+// `scheme` is a resolved variant (1, 2 or 3).  ev (optional, 2*iterations+1 events): kernel boundaries, for
+// the per-kernel timing of PN_OPT_PROFILE (scheme 3: the second interval of every iteration is empty).
+cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int scheme, cudaStream_t st,
                             int* launches, cudaEvent_t* ev) {
     const int nvec = (int)(g.npad / 4);
     const int nb = grid_for(nvec);
-    bool use_tma = variant == 2 || (variant == 0 && g.npad >= (1ll << 21));
     pn_tma_plan* plan = nullptr;
-    if (use_tma && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) {
-        if (variant == 2) return cudaErrorNotSupported;   // asked for explicitly: fail loudly
-        use_tma = false;
-    }
-    // ev (optional, 2*iterations+1 events): kernel boundaries, for the per-kernel timing of PN_OPT_PROFILE
+    pn_fused_plan* fplan = nullptr;
+    if (scheme == 2 && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) return cudaErrorNotSupported;
+    if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);
     for (int it = 0; it < iterations && e == cudaSuccess; ++it) {
-        if (use_tma) e = pn_launch_stencil_tma(plan, g, P, st);
+        if (scheme == 3) e = pn_launch_cg_fused(fplan, g, P, st);
+        else if (scheme == 2) e = pn_launch_stencil_tma(plan, g, P, st);
         else k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2);
         if (ev) cudaEventRecord(ev[2 * it + 1], st);
-        k_update<<<nb, TPB, 0, st>>>(nvec, P);
+        if (scheme != 3) k_update<<<nb, TPB, 0, st>>>(nvec, P);
         if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
     pn_tma_plan_free(plan);
-    *launches += 2 * iterations;
+    pn_fused_plan_free(fplan);
+    *launches += (scheme == 3 ? 1 : 2) * iterations;
     return e != cudaSuccess ? e : cudaGetLastError();
 }

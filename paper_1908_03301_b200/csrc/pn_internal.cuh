@@ -112,6 +112,7 @@ struct pn_ptrs {
     float* s;                   // s_i = 1/sqrt(diag_i) on solved nodes, 0 elsewhere
     double* x64;                // pressures (fp64), all nodes
     float *r, *p, *p2, *q, *xh; // fp32 CG vectors of the scaled system (p, p2: double-buffered search direction)
+    float *r2, *q2;             // second buffers of r and q for the single-kernel iteration (pn_fused_tma.cu)
     signed char* cls;           // node classes
     int* parent;                // union-find forest (aliases q)
     int* flags;                 // per-root inlet/outlet contact bits (aliases xh)
@@ -125,7 +126,7 @@ int pn_sm_count();
 cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, int x0_linear, cudaStream_t st,
                             int* launches);
-cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches);
 cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,
                                 double delta2, int max_iters, int reset_iters, cudaStream_t st, int* launches);
@@ -135,6 +136,16 @@ cudaError_t pn_launch_flux(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, 
 cudaError_t pn_launch_export_x(const pn_geom& g, const pn_ptrs& P, double* out, cudaStream_t st, int* launches);
 cudaError_t pn_launch_export_cls(const pn_geom& g, const pn_ptrs& P, signed char* out, int user_dir_is_2d,
                                  cudaStream_t st, int* launches);
+
+// Single-kernel CG iteration, TMA-fed (pn_fused_tma.cu): S4 + S5 + S6 in one launch
+struct pn_fused_plan;
+bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P);
+void pn_fused_plan_free(pn_fused_plan* pl);
+cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
+
+// Which iteration scheme a PN_OPT_KERNEL value selects on this lattice: 1 = reference two-kernel,
+// 2 = two-kernel with the TMA S4 kernel, 3 = single fused TMA kernel
+int pn_resolve_variant(const pn_geom& g, int variant);
 
 // TMA-fed S4 kernel (pn_stencil_tma.cu)
 struct pn_tma_plan;

@@ -25,10 +25,12 @@ int grid_for(long long work_items) {
 // x64 carries the Dirichlet and pin values on the nodes that are not unknowns, so
 // (b - A x)_i = sum_j g_ij (x_j - x_i) over all six neighbours.  acc[0] = ||r||^2, acc[1] = ||r_hat||^2
 // (of the rounded fp32 values, i.e. exactly what the inner recurrence starts from).
-__global__ void k_residual64(pn_geom g, pn_ptrs P) {
+// `fused`: the single-kernel iteration double-buffers r; the next kernel reads buffer (iters & 1).
+__global__ void k_residual64(pn_geom g, pn_ptrs P, int fused) {
     __shared__ double sm[32];
     __shared__ double tot[2];
     double a0 = 0.0, a1 = 0.0;
+    float* __restrict__ rdst = (fused && (P.st->iters & 1)) ? P.r2 : P.r;
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const float s = P.s[n];
         float rh = 0.f;
@@ -44,7 +46,7 @@ __global__ void k_residual64(pn_geom g, pn_ptrs P) {
             a0 += r * r;
             a1 += (double)rh * (double)rh;
         }
-        P.r[n] = rh;
+        rdst[n] = rh;
     }
     a0 = pn_block_sum(a0, sm);
     a1 = pn_block_sum(a1, sm);
@@ -125,8 +127,8 @@ __global__ void k_export_cls(pn_geom g, const signed char* __restrict__ cls, sig
 
 }  // namespace
 
-cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_residual64<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches) {
+    k_residual64<<<grid_for(g.npad), TPB, 0, st>>>(g, P, fused);
     ++*launches;
     return cudaGetLastError();
 }

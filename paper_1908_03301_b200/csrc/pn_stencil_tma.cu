@@ -17,14 +17,13 @@
 //   * p.Ap is reduced warp -> block -> grid (last block done), alpha stays on the device.
 // HBM bytes per node: reads r, p, x_hat, wx, wy, wz (24 B) + writes p, q, x_hat (12 B) = 36 B, plus
 // the tile halo (2 rows in TY, 2 planes in the z chunk) which mostly hits L2.
-#include <cuda.h>  // CUtensorMap and enums only: the encoder is fetched with cudaGetDriverEntryPoint
 #include <new>
 
-#include "pn_internal.cuh"
+#include "pn_tma.cuh"
 
 namespace {
 
-constexpr int a32(int x) { return (x + 31) / 32 * 32; }  // TMA destinations: 128-byte (32-float) aligned
+using namespace pn_tma;
 
 template <int NBX_, int TY_, bool HAS_Y_, int S_>
 struct Cfg {
@@ -63,46 +62,6 @@ struct alignas(64) pn_tmaps {
     CUtensorMap r_main, r_slv, p_main[2], p_slv[2], xh, wx_main, wx_slv, wy, wz;
 };
 
-// ---- PTX wrappers ---------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
-    const uint32_t a = smem_u32(bar);
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(done)
-            : "r"(a), "r"(parity)
-            : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void tma_load_3d(float* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-            smem_u32(dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void bar_consumers(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
-
-__device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-__device__ __forceinline__ float4 fma4(float a, const float4& x, const float4& y) {
-    return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
-}
-
 // epilogue shared with the reference kernel (pn_inner.cu keeps its own copy: same arithmetic)
 __device__ __forceinline__ void finish_A(pn_state* st, double pq) {
     st->pq = pq;
@@ -134,8 +93,7 @@ k_stencil_tma(const __grid_constant__ pn_tmaps maps, pn_geom g, pn_ptrs P, int n
             mbar_init(full + s, 1);
             mbar_init(empty + s, C::NCONS / 32);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
 
@@ -299,36 +257,7 @@ k_stencil_tma(const __grid_constant__ pn_tmaps maps, pn_geom g, pn_ptrs P, int n
     }
 }
 
-// ---- host side: tensor maps ------------------------------------------------------------------------
-typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-encode_fn get_encoder() {
-    static encode_fn fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (encode_fn)p;
-    }
-    return fn;
-}
-
-// 3D map over a padded lattice array INCLUDING its two halo planes: dims (px, ny, nz + 2).
-bool make_map(CUtensorMap* m, const pn_geom& g, const float* base_with_halo, int bx, int by) {
-    encode_fn enc = get_encoder();
-    if (!enc) return false;
-    const cuuint64_t dims[3] = {(cuuint64_t)g.px, (cuuint64_t)g.ny, (cuuint64_t)g.nz + 2};
-    const cuuint64_t strides[2] = {(cuuint64_t)g.px * 4, (cuuint64_t)g.plane * 4};
-    const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
-    const cuuint32_t es[3] = {1, 1, 1};
-    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base_with_halo, dims, strides, box, es,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
+// ---- host side ----------------------------------------------------------------------------------------
 template <class C>
 bool build_maps(pn_tmaps* M, const pn_geom& g, const pn_ptrs& P) {
     const long long h = g.plane;
@@ -347,22 +276,6 @@ bool build_maps(pn_tmaps* M, const pn_geom& g, const pn_ptrs& P) {
     return ok;
 }
 
-// z-chunk length: balance the persistent grid against the two extra r/p planes every chunk costs
-int choose_lz(int nz, int tiles, int nblocks) {
-    int best = 1;
-    double best_eff = 0.0;
-    for (int lz = 4; lz <= 64; ++lz) {
-        const int chunks = (nz + lz - 1) / lz;
-        const long long items = (long long)chunks * tiles;
-        const long long rounds = (items + nblocks - 1) / nblocks;
-        const double balance = (double)items / (double)(rounds * nblocks);
-        const double halo = 36.0 / (36.0 + 16.0 / lz);
-        const double eff = balance * halo;
-        if (eff > best_eff + 1e-9) { best_eff = eff; best = lz; }
-    }
-    return best;
-}
-
 template <class C>
 cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_tmaps& M, cudaStream_t st) {
     static bool attr_done = false;
@@ -373,7 +286,7 @@ cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_tmaps& M, cu
     }
     const int ntx = (g.px + C::TXW - 1) / C::TXW, nty = (g.ny + C::TY - 1) / C::TY;
     const int sms = pn_sm_count();
-    const int lz = choose_lz(g.nz, ntx * nty, sms);
+    const int lz = choose_lz(g.nz, ntx * nty, sms, 36.0, 16.0);
     const int nchunks = (g.nz + lz - 1) / lz;
     const long long total = (long long)ntx * nty * nchunks;
     const int nb = (int)(total < sms ? total : sms);

@@ -111,9 +111,10 @@ def test_cfg4_sibling_128(pn, oracle):
 @pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 31, 7), (130, 6, 3)])
 @pytest.mark.parametrize("direction", [0, 1, 2])
 @pytest.mark.parametrize("p", [1.0, 0.6])
-@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
 def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
-    """kernel 1 = reference S4 kernel, 2 = TMA-fed 2.5D kernel (forced, whatever the size)."""
+    """kernel 1 = reference two-kernel iteration, 2 = TMA-fed 2.5D S4 kernel + S5 kernel, 3 = single fused TMA
+    kernel per iteration (2 and 3 forced, whatever the size)."""
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(*shape, seed=7 + direction, p=p)
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
@@ -122,30 +123,32 @@ def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
 @pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (3, 64), (257, 31)])
 @pytest.mark.parametrize("direction", [0, 1])
 @pytest.mark.parametrize("p", [1.0, 0.7])
-@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
 def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(shape[0], shape[1], 1, seed=11 + direction, p=p)
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
+@pytest.mark.parametrize("kernel", [2, 3])
 @pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
-def test_tma_kernel_multi_tile(pn, oracle, shape, direction):
+def test_tma_kernel_multi_tile(pn, oracle, shape, direction, kernel):
     """Lattices wider than one 256-node TMA box and taller than one 8-row tile: x and y halos between
     tiles, several z chunks, ragged tails in all three directions."""
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(*shape, seed=5, p=0.75)
-    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 2})
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-def test_tma_kernel_2d_wide(pn, oracle):
+@pytest.mark.parametrize("kernel", [2, 3])
+def test_tma_kernel_2d_wide(pn, oracle, kernel):
     """2D lattice wider than the 2048-node tile of the 2D configuration (x halo between tiles)."""
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(2100, 40, 1, seed=9, p=1.0)
-    compare(pn, oracle, net, 1, opts={pn.PN_OPT_KERNEL: 2})
+    compare(pn, oracle, net, 1, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
 def test_kernel_variants(pn, oracle, kernel):
     """Both S4 kernels must pass the same parity bar (0 = automatic choice is what the other tests use)."""
     from paper_1908_03301_b200 import inputs
@@ -159,6 +162,8 @@ def test_zero_start_and_restart_options(pn, oracle):
     net = inputs.cfg3_percolation_3d(32, 32, 32)
     compare(pn, oracle, net, 0, opts={pn.PN_OPT_X0: 0})
     compare(pn, oracle, net, 0, opts={pn.PN_OPT_DELTA: 0.01, pn.PN_OPT_CHUNK: 7})
+    compare(pn, oracle, net, 0, opts={pn.PN_OPT_X0: 0, pn.PN_OPT_KERNEL: 3})
+    compare(pn, oracle, net, 0, opts={pn.PN_OPT_DELTA: 0.01, pn.PN_OPT_CHUNK: 7, pn.PN_OPT_KERNEL: 3})
 
 
 # ---- closed forms straight on the GPU path (also pins of the oracle, see test_oracle_pins.py) ----
@@ -311,18 +316,20 @@ def test_error_paths(pn):
 def test_max_iters_status(pn):
     from paper_1908_03301_b200 import inputs
     net = inputs.cfg2_fbm_2d(128, 128)
-    info, *_ = gpu_solve(pn, net, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40})
-    assert info.status == pn.PN_MAX_ITERS
-    assert 40 <= info.inner_iters <= 40 + 64
-    assert info.rel_residual > 1e-12
+    for kernel in (1, 3):
+        info, *_ = gpu_solve(pn, net, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40, pn.PN_OPT_KERNEL: kernel})
+        assert info.status == pn.PN_MAX_ITERS
+        assert 40 <= info.inner_iters <= 40 + 64
+        assert info.rel_residual > 1e-12
 
 
 def test_deterministic(pn):
     """Fixed-order grid reductions: two solves of the same input agree bit for bit."""
     from paper_1908_03301_b200 import inputs
     net = inputs.cfg3_percolation_3d(40, 40, 40)
-    a = gpu_solve(pn, net, 0, 1e-10)
-    b = gpu_solve(pn, net, 0, 1e-10)
-    assert a[0].inner_iters == b[0].inner_iters
-    assert np.array_equal(a[1], b[1])
-    assert a[3] == b[3]
+    for kernel in (1, 3):
+        a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel})
+        b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel})
+        assert a[0].inner_iters == b[0].inner_iters
+        assert np.array_equal(a[1], b[1])
+        assert a[3] == b[3]
