@@ -61,16 +61,19 @@ typedef struct {
     int status;            /* the code pn_solve returned                                            */
     int outer_cycles;      /* fp64 true-residual evaluations  r = b - A x  (S8(a) S3)                */
     int inner_iters;       /* fp32 CG iterations (S8(a) S4+S5), summed over the solve               */
-    int reserved;
+    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 2 or 3) */
     double rel_residual;   /* true fp64 ||b - A x||_2 / ||b||_2 over the solved nodes at exit       */
     double b_norm;         /* ||b||_2 of the zero-initial-guess system (S8(c) reading 5)            */
     long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
     double t_label_ms;     /* S1 + set-up (labelling, pruning, scaling), device time                */
     double t_solve_ms;     /* S3..S7 loop, device time                                              */
-    double t_stencil_ms;   /* with PN_OPT_PROFILE: summed device time of the S4 kernel launches ...  */
+    double t_stencil_ms;   /* with PN_OPT_PROFILE: summed device time of the S4 kernel launches (scheme 3:
+                              of the single fused S4+S5+S6 kernel; t_update_ms is then 0) ...       */
     double t_update_ms;    /* ... and of the S5 kernel launches (CUDA events on the handle's stream) */
     int n_timed_iters;     /* ... over this many inner iterations                                   */
     int reserved2;
+    long long n_peeled;    /* solved nodes taken out of the system as dangling ends (PN_OPT_PEEL) and
+                              back-filled after the solve; they are counted in n_solved too           */
 } pn_info;
 
 /* options for pn_set_option */
@@ -80,7 +83,9 @@ enum {
                                recursive residual has fallen by this factor since the last one
                                (default 0.1; S8(c) reading 4)                                       */
     PN_OPT_X0 = 2,          /* initial guess on solved nodes: 0 = zero, 1 = linear profile along the
-                               solve axis (default 1; S8(c) reading 6)                              */
+                               solve axis (default 1; S8(c) reading 6), 2 = warm start: the pressures
+                               this handle's previous solve left (S8(f) item 4: re-solves after a
+                               change of conductances or direction; first solve: same as 1)         */
     PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32)            */
     PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
@@ -88,8 +93,13 @@ enum {
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept for cross-checks and small lattices), 2 = TMA-fed 2.5D S4 kernel
                                + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused)      */
-    PN_OPT_PROFILE = 6      /* 1: record CUDA events around every S4 / S5 launch and report the
+    PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
+    PN_OPT_PEEL = 7         /* 1 (default): dead-end peeling -- solved nodes left with one open bond
+                               carry no current (S8(c) reading 7, S8(f) item 1); they are removed from the
+                               system, recursively, and take the pressure of the node they hang from
+                               after the solve.  Pressures of all nodes stay those of the full system.
+                               0: keep them as unknowns                                             */
 };
 
 /* Device bytes pn_create needs for an nx x ny x nz lattice (0 on a bad shape). */

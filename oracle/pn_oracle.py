@@ -172,6 +172,51 @@ def classify(nx, ny, nz, g64, direction):
 
 
 # --------------------------------------------------------------------------------------------------
+# dead ends inside the spanning clusters (S8c reading 7, S8(f) item 1)
+# --------------------------------------------------------------------------------------------------
+def dangling_ends(nx, ny, nz, g64, classes):
+    """Boolean mask (nz, ny, nx) of the SOLVED nodes that are dangling (tree-like dead) ends.
+
+    Definition (S8c reading 7: "dangling branches inside a spanning cluster have well-defined pressures
+    ... tree ends carrying no flow"): strip, one at a time and until none is left, any SOLVED node that has
+    exactly ONE open bond to a node that is still present (present = SOLVED and not yet stripped, or on a
+    Dirichlet plane).  What remains is the 2-core of the spanning clusters with the Dirichlet nodes kept;
+    the stripped nodes carry no current and sit at the pressure of the node their tree hangs from.
+    These nodes STAY unknowns of the oracle's linear system; this mask only says which ones a solver may
+    remove and back-fill.  Serial work-list implementation."""
+    gx, gy, gz = g64
+    N = nx * ny * nz
+    cls = classes.ravel().tolist()
+    fl = (gx.ravel().tolist(), gy.ravel().tolist(), gz.ravel().tolist())
+    stride = (1, nx, nx * ny)
+    dims = (nx, ny, nz)
+    present = [c in (INLET, OUTLET, SOLVED) for c in cls]
+
+    def open_neighbours(n):
+        c = (n % nx, (n // nx) % ny, n // (nx * ny))
+        out = []
+        for a in range(3):
+            if c[a] + 1 < dims[a] and fl[a][n] > 0.0 and present[n + stride[a]]:
+                out.append(n + stride[a])
+            if c[a] > 0 and fl[a][n - stride[a]] > 0.0 and present[n - stride[a]]:
+                out.append(n - stride[a])
+        return out
+
+    stripped = [False] * N
+    work = deque(n for n in range(N) if cls[n] == SOLVED)
+    while work:
+        n = work.popleft()
+        if stripped[n] or cls[n] != SOLVED:
+            continue
+        nb = open_neighbours(n)
+        if len(nb) == 1 and cls[nb[0]] == SOLVED:
+            stripped[n] = True
+            present[n] = False
+            work.append(nb[0])
+    return np.asarray(stripped, dtype=bool).reshape(nz, ny, nx)
+
+
+# --------------------------------------------------------------------------------------------------
 # step 4: assembled sparse Laplacian over the solved nodes
 # --------------------------------------------------------------------------------------------------
 def assemble(nx, ny, nz, g64, classes):

@@ -30,10 +30,10 @@ struct pn_ctx {
     float* raw_store[3];
     pn_state* h_state;          // pinned mirror
     cudaEvent_t ev[4];
-    bool have_g, have_solution;
+    bool have_g, have_solution, ever_solved;
     int last_dir_user;
     // options
-    int max_iters, chunk, x0_linear, skip_label, variant, profile;
+    int max_iters, chunk, x0_linear, skip_label, variant, profile, peel;
     cudaEvent_t* pev;           // event pool for PN_OPT_PROFILE (2*chunk+1), created on demand
     int pev_n;
     double delta;
@@ -146,7 +146,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 1;
     ctx->delta = 0.1;
     ctx->last_dir_user = -1;
     cudaDeviceProp prop;
@@ -205,11 +205,12 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
     switch (key) {
         case PN_OPT_MAX_ITERS: if (value < 1 || value > 2e9) return PN_ERR_ARG; ctx->max_iters = (int)value; return PN_OK;
         case PN_OPT_DELTA: if (!(value > 0.0 && value < 1.0)) return PN_ERR_ARG; ctx->delta = value; return PN_OK;
-        case PN_OPT_X0: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
+        case PN_OPT_X0: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
         case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
         case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
+        case PN_OPT_PEEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
 }
@@ -291,13 +292,15 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
 
     // ---- S1 + set-up ----
     CK(cudaEventRecord(ctx->ev[0], s));
-    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + sizeof(P.st->count), s));
+    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + sizeof(P.st->count) + sizeof(P.st->n_peeled), s));
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     const int scheme = pn_resolve_variant(g, ctx->variant);
     const int fused = scheme == 3;
     const bool do_label = !ctx->skip_label && ctx->h_state->any_closed;
-    CK(pn_launch_label(g, P, do_label, ctx->x0_linear, s, &nl));
+    const bool do_peel = do_label && ctx->peel;
+    const int x0_mode = (ctx->x0_linear == 2 && !ctx->ever_solved) ? 1 : ctx->x0_linear;   // nothing to warm-start from yet
+    CK(pn_launch_label(g, P, do_label, do_peel, x0_mode, s, &nl));
     // parent / flags aliased q / x_hat: clear the CG vectors before the first iteration
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
@@ -313,6 +316,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     if (rc) return rc;
     pn_state* h = ctx->h_state;
     const long long n_solved = (long long)h->count[0];
+    const long long n_peeled = (long long)h->n_peeled;
     const double nb = sqrt(h->acc[2]);
     double rn = sqrt(h->acc[0]);
     double rr_hat = h->acc[1];
@@ -385,22 +389,26 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
             CK(pn_launch_set_state(P, rr_hat, beta, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 0, s, &nl));
         }
     }
+    if (n_peeled > 0) CK(pn_launch_backfill(g, P, s, &nl));   // dangling ends take the pressure of the node they hang from
     CK(cudaEventRecord(ctx->ev[2], s));
     CK(cudaStreamSynchronize(s));
     ctx->launches += nl;
     ctx->have_solution = true;
+    ctx->ever_solved = true;
     ctx->last_dir_user = direction;
     if (info) {
         float ms = 0.f;
         info->status = status;
         info->outer_cycles = outer;
         info->inner_iters = total_iters;
+        info->kernel_scheme = scheme;
         info->rel_residual = nb > 0.0 ? rn / nb : 0.0;
         info->b_norm = nb;
         info->n_solved = n_solved;
         info->n_inlet_only = (long long)h->count[1];
         info->n_outlet_only = (long long)h->count[2];
         info->n_floating = (long long)h->count[3];
+        info->n_peeled = n_peeled;
         if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
         if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
         info->t_stencil_ms = t_stencil;

@@ -18,6 +18,8 @@
 
 #define PN_MAX_BLOCKS 2048      // upper bound on gridDim.x of every reducing kernel (partial slots)
 #define PN_CLASS_PAD 7          // internal: pad column (never exported)
+#define PN_CLASS_PEELED 8       // internal: 8 + c = solved node peeled off as a dangling end, hanging from its
+                                // neighbour in direction c (0:+x 1:-x 2:+y 3:-y 4:+z 5:-z); exported as SOLVED
 
 struct pn_geom {
     int nx, ny, nz;             // INTERNAL lattice dims (2D user lattices: ny = 1, nz = user ny)
@@ -43,6 +45,7 @@ struct pn_state {
     double delta2;              // reliable-update threshold squared
     double acc[4];              // results of the fp64 reductions (residual norms, b norm, flux)
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
+    unsigned long long n_peeled;// solved nodes removed from the system as dangling ends (back-filled after the solve)
     int flag;                   // 0 run, 1 proxy-converged, 2 reliable update due, 3 breakdown, 4 budget
     int iters;                  // inner iterations done in this solve
     int max_iters;
@@ -115,7 +118,7 @@ struct pn_ptrs {
     float *r2, *q2;             // second buffers of r and q for the single-kernel iteration (pn_fused_tma.cu)
     signed char* cls;           // node classes
     int* parent;                // union-find forest (aliases q)
-    int* flags;                 // per-root inlet/outlet contact bits (aliases xh)
+    int* flags;                 // per-root inlet/outlet contact bits (aliases xh); after S1d: live bond degree (peeling)
     double* slots;              // 4 x PN_MAX_BLOCKS partial sums
     pn_state* st;
     void* scratch;              // export staging (aliases p, p2)
@@ -124,8 +127,9 @@ struct pn_ptrs {
 int pn_sm_count();
 
 cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
-cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, int x0_linear, cudaStream_t st,
-                            int* launches);
+cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, bool do_peel, int x0_linear,
+                            cudaStream_t st, int* launches);
+cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches);
 cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,

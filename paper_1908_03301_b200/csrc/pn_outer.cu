@@ -121,7 +121,8 @@ __global__ void k_export_x(pn_geom g, const double* __restrict__ x64, double* __
 __global__ void k_export_cls(pn_geom g, const signed char* __restrict__ cls, signed char* __restrict__ out) {
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.n; n += (long long)gridDim.x * blockDim.x) {
         const long long row = n / g.nx;
-        out[n] = cls[row * g.px + (n - row * g.nx)];
+        const signed char c = cls[row * g.px + (n - row * g.nx)];
+        out[n] = c >= PN_CLASS_PEELED ? (signed char)PN_CLASS_SOLVED : c;   // peeled dangling ends are solved nodes
     }
 }
 

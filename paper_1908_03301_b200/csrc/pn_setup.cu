@@ -133,6 +133,8 @@ __global__ void k_touch(pn_geom g, pn_ptrs P) {
 }
 
 // ---- S1d: node classes, class counts, pin values and the initial guess --------------------------
+// x0_linear: 0 = zero, 1 = linear profile along the solve axis, 2 = warm start (keep what x64 holds on the
+// solved nodes: the previous solve's pressures)
 template <bool LABEL>
 __global__ void k_classify(pn_geom g, pn_ptrs P, int x0_linear) {
     unsigned long long cnt[4] = {0, 0, 0, 0};
@@ -147,7 +149,10 @@ __global__ void k_classify(pn_geom g, pn_ptrs P, int x0_linear) {
             else {
                 int f = 3;
                 if (LABEL) f = __ldcg(P.flags + uf_find(P.parent, (int)n));
-                if (f == 3) { cls = PN_CLASS_SOLVED; x = x0_linear ? 1.0 - (double)ca / (double)(g.n_a - 1) : 0.0; cnt[0]++; }
+                if (f == 3) { cls = PN_CLASS_SOLVED; const double lin = 1.0 - (double)ca / (double)(g.n_a - 1);
+                    x = x0_linear ? lin : 0.0;
+                    if (x0_linear == 2) { const double old = P.x64[n]; if (isfinite(old)) x = old; }
+                    cnt[0]++; }
                 else if (f == 1) { cls = PN_CLASS_INLET_ONLY; x = 1.0; cnt[1]++; }
                 else if (f == 2) { cls = PN_CLASS_OUTLET_ONLY; cnt[2]++; }
                 else { cls = PN_CLASS_FLOATING; cnt[3]++; }
@@ -183,6 +188,74 @@ __global__ void k_prune(pn_geom g, pn_ptrs P) {
             const bool keep1 = P.cls[n + stride[b]] <= PN_CLASS_SOLVED;
             if (!(keep0 && keep1)) P.gs[b][n] = 0.f;
         }
+    }
+}
+
+// ---- S1f: dead-end (leaf) peeling inside the spanning clusters (SURVEY.md 8(f) item 1, 8(c) reading 7) ----
+// A solved node with a single open bond carries no current: its pressure equals that of the node it hangs
+// from, and so on up the dangling tree.  Such nodes are taken out of the linear system (their bond is
+// zeroed in the solve copy, so the neighbour's diagonal no longer counts it) and back-filled after the
+// solve (k_backfill), which keeps the pressures of ALL nodes those of the full system.  Near the
+// percolation threshold about half of a spanning cluster is dangling ends; removing them is what shortens
+// the critical slow-down -- fewer unknowns and a better-conditioned operator.
+// Asynchronous peeling: live bond degrees in an int array; a thread that removes a leaf decrements the
+// neighbour's degree and, if that made the neighbour a leaf, carries on with it (no rounds, so a long
+// dangling chain costs one walk, not one launch per node).  A node is claimed with atomicCAS(deg, 1, 0).
+__global__ void k_degree(pn_geom g, pn_ptrs P) {
+    int* __restrict__ deg = P.flags;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        int d = 0;
+        if (P.cls[n] == PN_CLASS_SOLVED)
+            d = (P.gs[0][n] != 0.f) + (P.gs[0][n - 1] != 0.f) + (P.gs[1][n] != 0.f) + (P.gs[1][n - g.px] != 0.f) +
+                (P.gs[2][n] != 0.f) + (P.gs[2][n - g.plane] != 0.f);
+        deg[n] = d;
+    }
+}
+
+__global__ void k_peel(pn_geom g, pn_ptrs P) {
+    int* deg = P.flags;
+    const long long stride[3] = {1, g.px, g.plane};
+    unsigned long long cnt = 0;
+    for (long long n0 = blockIdx.x * (long long)blockDim.x + threadIdx.x; n0 < g.npad; n0 += (long long)gridDim.x * blockDim.x) {
+        long long n = n0;
+        while (__ldcg(deg + n) == 1 && atomicCAS(deg + n, 1, 0) == 1) {
+            // the one bond left (bonds zeroed by other threads are read at L2: their stores were fenced
+            // before the degree decrement that made this node a leaf)
+            int code = -1;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                if (__ldcg(P.gs[b] + n) != 0.f) code = 2 * b;
+                if (__ldcg(P.gs[b] + n - stride[b]) != 0.f) code = 2 * b + 1;
+            }
+            if (code < 0) break;
+            const long long sb = stride[code >> 1];
+            const long long m = (code & 1) ? n - sb : n + sb;
+            if (P.cls[m] != PN_CLASS_SOLVED) { deg[n] = 1; break; }   // hangs from a Dirichlet node: not a dead end
+            P.cls[n] = (signed char)(PN_CLASS_PEELED + code);
+            __stcg(P.gs[code >> 1] + ((code & 1) ? m : n), 0.f);
+            __threadfence();
+            ++cnt;
+            if (atomicSub(deg + m, 1) != 2) break;                   // the neighbour did not become a leaf
+            n = m;
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&P.st->n_peeled, cnt);
+}
+
+// After the solve: every peeled node takes the pressure of the unpeeled node its dangling tree hangs from.
+__global__ void k_backfill(pn_geom g, pn_ptrs P) {
+    const long long stride[3] = {1, g.px, g.plane};
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        int c = P.cls[n];
+        if (c < PN_CLASS_PEELED) continue;
+        long long m = n;
+        for (long long guard = 0; c >= PN_CLASS_PEELED && guard < g.npad; ++guard) {
+            const int code = c - PN_CLASS_PEELED;
+            m += (code & 1) ? -stride[code >> 1] : stride[code >> 1];
+            c = P.cls[m];
+        }
+        P.x64[n] = P.x64[m];
     }
 }
 
@@ -234,8 +307,8 @@ cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t 
     return cudaGetLastError();
 }
 
-cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, int x0_linear, cudaStream_t st,
-                            int* launches) {
+cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, bool do_peel, int x0_linear,
+                            cudaStream_t st, int* launches) {
     const int nb = grid_for(g.npad);
     k_solve_copy<<<nb, TPB, 0, st>>>(g, P);
     ++*launches;
@@ -245,6 +318,11 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, i
         k_classify<true><<<nb, TPB, 0, st>>>(g, P, x0_linear);
         k_prune<<<nb, TPB, 0, st>>>(g, P);
         *launches += 4;
+        if (do_peel) {
+            k_degree<<<nb, TPB, 0, st>>>(g, P);
+            k_peel<<<nb, TPB, 0, st>>>(g, P);
+            *launches += 2;
+        }
     } else {
         k_classify<false><<<nb, TPB, 0, st>>>(g, P, x0_linear);
         ++*launches;
@@ -252,5 +330,11 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, i
     k_scale<<<nb, TPB, 0, st>>>(g, P);
     k_weights<<<nb, TPB, 0, st>>>(g, P);
     *launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    k_backfill<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    ++*launches;
     return cudaGetLastError();
 }

@@ -333,3 +333,83 @@ def test_deterministic(pn):
         assert a[0].inner_iters == b[0].inner_iters
         assert np.array_equal(a[1], b[1])
         assert a[3] == b[3]
+
+
+# ---- dead-end peeling: integer work bit-exact, pressures of ALL nodes unchanged ----
+def _oracle_dangling(net, classes):
+    from oracle import pn_oracle as po
+    g64 = po.widen(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz)
+    return po.dangling_ends(net.nx, net.ny, net.nz, g64, classes)
+
+
+@pytest.mark.parametrize("maker,direction", [
+    (lambda i: i.cfg3_percolation_3d(64, 64, 64), 0), (lambda i: i.cfg3_percolation_3d(40, 33, 50), 2),
+    (lambda i: i.cfg4_fbm_cut_3d(48, 40, 36), 1), (lambda i: i.iid_diluted(150, 120, 1, seed=4, p=0.62), 0),
+    (lambda i: i.iid_diluted(150, 120, 1, seed=4, p=0.62), 1)])
+def test_peeling_count_and_parity(pn, oracle, maker, direction):
+    """The number of peeled nodes equals the oracle's serial leaf stripping (the 2-core is unique, so the
+    asynchronous GPU peeling must remove exactly the same set); pressures and G_eff pass the same parity bar with
+    and without peeling (peeled nodes are back-filled); peeling never costs iterations."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    on, P_on, fl_on, ref = compare(pn, oracle, net, direction, opts={pn.PN_OPT_PEEL: 1})
+    off, P_off, fl_off, _ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_PEEL: 0})
+    mask = _oracle_dangling(net, ref.classes)
+    assert on.n_peeled == int(mask.sum()) > 0
+    assert off.n_peeled == 0
+    assert on.n_solved == off.n_solved == ref.n_solved
+    assert on.inner_iters <= off.inner_iters
+    # a peeled node sits exactly at the pressure of some neighbour (the one it hangs from)
+    P = P_on
+    nb = np.full(P.shape, np.inf)
+    for ax in range(3):
+        for sh in (1, -1):
+            d = np.abs(P - np.roll(P, sh, axis=ax))
+            sl = [slice(None)] * 3
+            sl[ax] = 0 if sh == 1 else -1
+            d[tuple(sl)] = np.inf            # no wrap-around neighbours
+            nb = np.minimum(nb, d)
+    assert float(np.max(nb[mask])) == 0.0
+
+
+def test_peeling_long_chain(pn, oracle):
+    """A dangling chain of 300 nodes hanging from a uniform backbone: one asynchronous walk peels all of it."""
+    nx, ny = 304, 3
+    gx = np.zeros((1, ny, nx), dtype=np.float32)
+    gy = np.zeros((1, ny, nx), dtype=np.float32)
+    gx[0, 0, :nx - 1] = 1.0                  # backbone along the bottom row
+    gy[0, 0, 1] = 0.5                        # stub up from (1,0) ...
+    gy[0, 1, 1] = 0.5
+    gx[0, 2, 1:301] = 2.0                    # ... then 300 nodes along the top row
+    from paper_1908_03301_b200.inputs import Network
+    net = Network(nx, ny, 1, gx, gy, None, name="chain")
+    info, P, fl, ref = compare(pn, oracle, net, 0)
+    assert info.n_peeled == 302
+    assert np.all(P[0, 2, 1:302] == P[0, 0, 1])
+    assert fl[2] == pytest.approx(1.0 / (nx - 1), rel=1e-12)
+
+
+def test_warm_start(pn, oracle):
+    """PN_OPT_X0 = 2: re-solve after a small change of the conductances starting from the
+    previous pressures -- same parity bar, far fewer iterations than a cold solve."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg4_fbm_cut_3d(64, 64, 64)
+    rng = np.random.default_rng(8)
+    bump = lambda g: (g * (1.0 + 1e-5 * rng.standard_normal(g.shape))).astype(np.float32)   # zeros stay zero
+    gx2, gy2, gz2 = bump(net.gx), bump(net.gy), bump(net.gz)
+    ref = oracle.solve(net.nx, net.ny, net.nz, gx2, gy2, gz2, 0, 1e-13)
+    h = pn.Network(net.nx, net.ny, net.nz)
+    h.set_option(pn.PN_OPT_X0, 2)
+    h.set_conductances(net.gx, net.gy, net.gz)
+    first = h.solve(0, 1e-12)                          # nothing to start from: linear profile
+    h.set_conductances(gx2, gy2, gz2)
+    warm = h.solve(0, 1e-12)
+    P = h.pressures().cpu().numpy()
+    g_eff = h.flux()[2]
+    h.set_option(pn.PN_OPT_X0, 1)
+    cold = h.solve(0, 1e-12)
+    h.close()
+    assert np.max(np.abs(P - ref.P)) <= P_TOL
+    assert abs(g_eff - ref.g_eff) <= G_TOL * abs(ref.g_eff)
+    assert warm.inner_iters < 0.85 * cold.inner_iters
+    assert first.inner_iters == pytest.approx(cold.inner_iters, rel=0.1)

@@ -384,3 +384,92 @@ def test_residual_certificate_detects_a_wrong_field():
     bad[tuple(idx)] += 1e-6
     rel2, _ = po.residual_certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, bad, 0)
     assert rel2 > 1e-8
+
+
+# ---------------------------------------------------------------- dangling ends (S8c reading 7) ---
+def _open_nbrs(nx, ny, nz, g64, n):
+    """Open-bond neighbours of node n, written independently of the oracle (coordinate loops)."""
+    i, j, k = n % nx, (n // nx) % ny, n // (nx * ny)
+    out = []
+    for (di, dj, dk) in ((1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)):
+        a, b, c = i + di, j + dj, k + dk
+        if not (0 <= a < nx and 0 <= b < ny and 0 <= c < nz):
+            continue
+        arr = g64[0] if di else (g64[1] if dj else g64[2])
+        g = arr[min(k, c), min(j, b), min(i, a)]        # the forward bond lives on the lower-index end
+        if g > 0.0:
+            out.append(a + nx * (b + ny * c))
+    return out
+
+
+@pytest.mark.parametrize("shape,direction,p,seed", [((5, 4, 1), 0, 0.7, s) for s in range(6)] +
+                         [((4, 5, 1), 1, 0.75, s) for s in range(4)] + [((4, 3, 3), 0, 0.6, s) for s in range(6)])
+def test_dangling_ends_equal_complement_of_bruteforce_2core(shape, direction, p, seed):
+    """The nodes left after stripping are the 2-core (Dirichlet nodes kept): the UNION of all node subsets in
+    which every member keeps >= 2 open neighbours inside (subset + Dirichlet planes).  Enumerated outright."""
+    nx, ny, nz = shape
+    net = inputs.iid_diluted(nx, ny, nz, seed=100 + seed, p=p)
+    g64 = po.widen(nx, ny, nz, net.gx, net.gy, net.gz)
+    cls = po.classify(nx, ny, nz, g64, direction)
+    mask = po.dangling_ends(nx, ny, nz, g64, cls)
+    flat = cls.ravel()
+    solved = [n for n in range(nx * ny * nz) if flat[n] == po.SOLVED]
+    assert len(solved) <= 18
+    dirichlet = {n for n in range(nx * ny * nz) if flat[n] in (po.INLET, po.OUTLET)}
+    nbrs = {n: _open_nbrs(nx, ny, nz, g64, n) for n in solved}
+    core = set()
+    for bits in range(1 << len(solved)):
+        sub = {solved[t] for t in range(len(solved)) if bits >> t & 1}
+        keep = sub | dirichlet
+        if all(sum(m in keep for m in nbrs[n]) >= 2 for n in sub):
+            core |= sub
+    expect = np.zeros(nx * ny * nz, dtype=bool)
+    expect[[n for n in solved if n not in core]] = True
+    assert np.array_equal(mask.ravel(), expect)
+    assert not mask.ravel()[[n for n in range(nx * ny * nz) if flat[n] != po.SOLVED]].any()
+
+
+def test_dangling_ends_hand_built_stub():
+    """5 x 3 lattice, x direction: the middle row is the backbone; a two-node stub (2,2) -- (3,2) hangs from
+    (2,1).  Exactly those two nodes are dangling; they sit at the pressure of (2,1) = 1/2."""
+    nx, ny = 5, 3
+    gx = np.zeros((1, ny, nx), dtype=np.float32)
+    gy = np.zeros((1, ny, nx), dtype=np.float32)
+    gx[0, 1, :4] = 1.0           # backbone
+    gy[0, 1, 2] = 2.0            # (2,1) -- (2,2)
+    gx[0, 2, 2] = 3.0            # (2,2) -- (3,2)
+    g64 = po.widen(nx, ny, 1, gx, gy, None)
+    cls = po.classify(nx, ny, 1, g64, 0)
+    mask = po.dangling_ends(nx, ny, 1, g64, cls)
+    expect = np.zeros((1, ny, nx), dtype=bool)
+    expect[0, 2, 2] = expect[0, 2, 3] = True
+    assert np.array_equal(mask, expect)
+    res = po.solve(nx, ny, 1, gx, gy, None, 0, 1e-14)
+    assert res.P[0, 2, 2] == pytest.approx(0.5, abs=1e-13) and res.P[0, 2, 3] == pytest.approx(0.5, abs=1e-13)
+
+
+@pytest.mark.parametrize("direction", [0, 2])
+def test_dangling_ends_carry_no_current(direction):
+    """Physics pin: in the solution of the FULL system every bond at a dangling node carries zero current."""
+    net = inputs.iid_diluted(14, 12, 10, seed=41, p=0.36)
+    nx, ny, nz = net.nx, net.ny, net.nz
+    res = run(net, direction, tol=1e-14)
+    assert res.status == "ok"
+    g64 = po.widen(nx, ny, nz, net.gx, net.gy, net.gz)
+    mask = po.dangling_ends(nx, ny, nz, g64, res.classes)
+    assert 0 < mask.sum() < res.n_solved
+    P = res.P
+    cur = [np.zeros(P.shape) for _ in range(3)]
+    cur[0][:, :, :-1] = g64[0][:, :, :-1] * (P[:, :, 1:] - P[:, :, :-1])
+    cur[1][:, :-1, :] = g64[1][:, :-1, :] * (P[:, 1:, :] - P[:, :-1, :])
+    cur[2][:-1, :, :] = g64[2][:-1, :, :] * (P[1:, :, :] - P[:-1, :, :])
+    # only bonds between nodes of the solved system matter (pinned clusters are not connected to it)
+    worst = 0.0
+    for a, (sl_lo, sl_hi) in enumerate((((slice(None), slice(None), slice(0, -1)), (slice(None), slice(None), slice(1, None))),
+                                        ((slice(None), slice(0, -1), slice(None)), (slice(None), slice(1, None), slice(None))),
+                                        ((slice(0, -1), slice(None), slice(None)), (slice(1, None), slice(None), slice(None))))):
+        touched = mask[sl_lo] | mask[sl_hi]
+        worst = max(worst, float(np.max(np.abs(cur[a][sl_lo][touched]), initial=0.0)))
+    assert worst < 1e-11
+    # and some bond that is NOT at a dangling node does carry current
+    assert max(float(np.max(np.abs(c))) for c in cur) > 1e-3
