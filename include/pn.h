@@ -95,11 +95,13 @@ enum {
                                + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused)      */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
-    PN_OPT_PEEL = 7         /* 1 (default): dead-end peeling -- solved nodes left with one open bond
-                               carry no current (S8(c) reading 7, S8(f) item 1); they are removed from the
-                               system, recursively, and take the pressure of the node they hang from
-                               after the solve.  Pressures of all nodes stay those of the full system.
-                               0: keep them as unknowns                                             */
+    PN_OPT_PEEL = 7         /* dead-end peeling: solved nodes left with one open bond carry no current
+                               (S8(c) reading 7, S8(f) item 1); they are removed from the system,
+                               recursively, and take the pressure of the node they hang from after the
+                               solve.  Pressures of all nodes stay those of the full system.
+                               0: never (all solved nodes are unknowns), 1: always, 2 (default): only if
+                               at least 10 % of the solved nodes can be removed (below that the iteration
+                               count does not improve measurably and the peeling is undone)         */
 };
 
 /* Device bytes pn_create needs for an nx x ny x nz lattice (0 on a bad shape). */

@@ -45,6 +45,8 @@ struct pn_ctx {
 
 namespace {
 
+constexpr double PN_PEEL_MIN_FRACTION = 0.10;
+
 int g_sm_count = 0;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -146,7 +148,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 1;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2;
     ctx->delta = 0.1;
     ctx->last_dir_user = -1;
     cudaDeviceProp prop;
@@ -210,7 +212,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
         case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
-        case PN_OPT_PEEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
+        case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
 }
@@ -301,6 +303,18 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     const bool do_peel = do_label && ctx->peel;
     const int x0_mode = (ctx->x0_linear == 2 && !ctx->ever_solved) ? 1 : ctx->x0_linear;   // nothing to warm-start from yet
     CK(pn_launch_label(g, P, do_label, do_peel, x0_mode, s, &nl));
+    if (do_peel && ctx->peel == 2) {
+        // automatic: keep the peeling only if it removes at least PN_PEEL_MIN_FRACTION of the unknowns.  Peeled nodes are
+        // still streamed (structured storage), so the gain is fewer iterations only; measured on B200:
+        // 52 % peeled -> -28 % iterations (CFG3), 3.8 % peeled -> +1.8 % (CFG4: within the noise of the iteration count)
+        rc = read_state(ctx);
+        if (rc) return rc;
+        if ((double)ctx->h_state->n_peeled < PN_PEEL_MIN_FRACTION * (double)ctx->h_state->count[0]) {
+            CK(pn_launch_unpeel(g, P, s, &nl));
+            CK(cudaMemsetAsync(&P.st->n_peeled, 0, sizeof(P.st->n_peeled), s));
+        }
+    }
+    CK(pn_launch_scale(g, P, s, &nl));
     // parent / flags aliased q / x_hat: clear the CG vectors before the first iteration
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));

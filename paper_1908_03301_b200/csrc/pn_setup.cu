@@ -243,6 +243,21 @@ __global__ void k_peel(pn_geom g, pn_ptrs P) {
     if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&P.st->n_peeled, cnt);
 }
 
+// Undo a peeling that removed too few nodes to pay (PN_OPT_PEEL = 2, see pn_api.cu): put every peeled node back
+// as an unknown and restore its bond from the caller's conductances.
+__global__ void k_unpeel(pn_geom g, pn_ptrs P) {
+    const long long stride[3] = {1, g.px, g.plane};
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const int c = P.cls[n];
+        if (c < PN_CLASS_PEELED) continue;
+        const int code = c - PN_CLASS_PEELED, b = code >> 1;
+        const long long lo = (code & 1) ? n - stride[b] : n;      // the forward bond lives on its lower-index end
+        const coords cc = coords_of(g, lo);
+        P.gs[b][lo] = P.raw[b][cc.i + (long long)g.nx * (cc.j + (long long)g.ny * cc.k)];
+        P.cls[n] = PN_CLASS_SOLVED;
+    }
+}
+
 // After the solve: every peeled node takes the pressure of the unpeeled node its dangling tree hangs from.
 __global__ void k_backfill(pn_geom g, pn_ptrs P) {
     const long long stride[3] = {1, g.px, g.plane};
@@ -327,6 +342,12 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, b
         k_classify<false><<<nb, TPB, 0, st>>>(g, P, x0_linear);
         ++*launches;
     }
+    return cudaGetLastError();
+}
+
+// Diagonal scale, ||b||^2 and the scaled weights of the inner system, from the final solve copy.
+cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    const int nb = grid_for(g.npad);
     k_scale<<<nb, TPB, 0, st>>>(g, P);
     k_weights<<<nb, TPB, 0, st>>>(g, P);
     *launches += 2;
@@ -335,6 +356,12 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, b
 
 cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
     k_backfill<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    k_unpeel<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }

@@ -349,7 +349,8 @@ def _oracle_dangling(net, classes):
 def test_peeling_count_and_parity(pn, oracle, maker, direction):
     """The number of peeled nodes equals the oracle's serial leaf stripping (the 2-core is unique, so the
     asynchronous GPU peeling must remove exactly the same set); pressures and G_eff pass the same parity bar with
-    and without peeling (peeled nodes are back-filled); peeling never costs iterations."""
+    and without peeling (peeled nodes are back-filled).  The iteration count is NOT guaranteed to fall (measured at
+    512^3 on CFG4: 3.8 % peeled, +1.8 % iterations); only a gross regression is checked here."""
     from paper_1908_03301_b200 import inputs
     net = maker(inputs)
     on, P_on, fl_on, ref = compare(pn, oracle, net, direction, opts={pn.PN_OPT_PEEL: 1})
@@ -358,7 +359,7 @@ def test_peeling_count_and_parity(pn, oracle, maker, direction):
     assert on.n_peeled == int(mask.sum()) > 0
     assert off.n_peeled == 0
     assert on.n_solved == off.n_solved == ref.n_solved
-    assert on.inner_iters <= off.inner_iters
+    assert on.inner_iters <= 1.1 * off.inner_iters
     # a peeled node sits exactly at the pressure of some neighbour (the one it hangs from)
     P = P_on
     nb = np.full(P.shape, np.inf)
@@ -413,3 +414,20 @@ def test_warm_start(pn, oracle):
     assert abs(g_eff - ref.g_eff) <= G_TOL * abs(ref.g_eff)
     assert warm.inner_iters < 0.85 * cold.inner_iters
     assert first.inner_iters == pytest.approx(cold.inner_iters, rel=0.1)
+
+
+def test_peeling_automatic_policy(pn, oracle):
+    """PN_OPT_PEEL = 2 (the default): the peeling is kept when it removes >= 10 % of the solved nodes (CFG3-like,
+    52 %) and undone below that (CFG4-like, 6 %) -- k_unpeel must restore the solve copy exactly, so the solve is
+    bit-identical to one that never peeled."""
+    from paper_1908_03301_b200 import inputs
+    near = inputs.cfg3_percolation_3d(64, 64, 64)
+    info, P, fl, ref = compare(pn, oracle, near, 0)                      # default options
+    assert info.n_peeled == int(_oracle_dangling(near, ref.classes).sum()) >= 0.1 * info.n_solved
+    far = inputs.cfg4_fbm_cut_3d(64, 64, 64)
+    auto, P_auto, fl_auto, ref = compare(pn, oracle, far, 0)
+    mask = _oracle_dangling(far, ref.classes)
+    assert 0 < int(mask.sum()) < 0.1 * auto.n_solved and auto.n_peeled == 0
+    never, P_never, fl_never, _ = compare(pn, oracle, far, 0, opts={pn.PN_OPT_PEEL: 0})
+    assert auto.inner_iters == never.inner_iters
+    assert np.array_equal(P_auto, P_never) and fl_auto == fl_never
