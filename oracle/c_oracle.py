@@ -65,12 +65,12 @@ def _load():
         _lib = ctypes.CDLL(build())
         fp = ctypes.POINTER(ctypes.c_float)
         dp = ctypes.POINTER(ctypes.c_double)
-        _lib.pno_solve.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, ctypes.c_double,
+        _lib.pno_solve.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                                         ctypes.c_int, ctypes.c_int, dp,
                                                         ctypes.POINTER(ctypes.c_byte),
                                                         ctypes.POINTER(_Info)]
         _lib.pno_solve.restype = ctypes.c_int
-        _lib.pno_certificate.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, dp, dp, dp,
+        _lib.pno_certificate.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, ctypes.c_int, dp, dp, dp,
                                          ctypes.POINTER(ctypes.c_byte)]
         _lib.pno_certificate.restype = ctypes.c_int
     return _lib
@@ -91,14 +91,14 @@ def _prep(nx, ny, nz, g):
 _STATUS = {0: "ok", 1: "no_spanning_cluster", 2: "max_iters"}
 
 
-def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, threads=0):
+def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, threads=0, periodic=False):
     lib = _load()
     gx, gy, gz = (_prep(nx, ny, nz, g) for g in (gx, gy, gz))
     P = np.empty((nz, ny, nx), dtype=np.float64)
     cls = np.empty((nz, ny, nx), dtype=np.int8)
     info = _Info()
     rc = lib.pno_solve(nx, ny, nz, _ptr(gx, ctypes.c_float), _ptr(gy, ctypes.c_float),
-                       _ptr(gz, ctypes.c_float), direction, tol, max_iter, threads,
+                       _ptr(gz, ctypes.c_float), direction, 1 if periodic else 0, tol, max_iter, threads,
                        _ptr(P, ctypes.c_double), _ptr(cls, ctypes.c_byte), ctypes.byref(info))
     if rc < 0:
         raise ValueError(f"pno_solve failed with code {rc}")
@@ -108,7 +108,7 @@ def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, threa
                          info.t_label, info.t_assemble, info.t_pcg, info.nnz)
 
 
-def certificate(nx, ny, nz, gx, gy, gz, P, direction=0, classes_out=None):
+def certificate(nx, ny, nz, gx, gy, gz, P, direction=0, classes_out=None, periodic=False):
     """(rel_residual, pin_err) of any pressure field; `classes_out` (int8 array of N entries, optional)
     receives the node classes of the serial labelling."""
     lib = _load()
@@ -117,7 +117,7 @@ def certificate(nx, ny, nz, gx, gy, gz, P, direction=0, classes_out=None):
     rel = ctypes.c_double()
     pin = ctypes.c_double()
     rc = lib.pno_certificate(nx, ny, nz, _ptr(gx, ctypes.c_float), _ptr(gy, ctypes.c_float),
-                             _ptr(gz, ctypes.c_float), direction, _ptr(P, ctypes.c_double),
+                             _ptr(gz, ctypes.c_float), direction, 1 if periodic else 0, _ptr(P, ctypes.c_double),
                              ctypes.byref(rel), ctypes.byref(pin), _ptr(classes_out, ctypes.c_byte))
     if rc < 0:
         raise ValueError(f"pno_certificate failed with code {rc}")

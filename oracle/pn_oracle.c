@@ -48,6 +48,7 @@ typedef struct {
     int nx, ny, nz, dir;
     long long N, stride[3];
     int dims[3];
+    int wrap[3]; /* lateral axis wraps around (periodic side faces); never the solve axis */
     const float *g[3];
 } lattice;
 
@@ -62,6 +63,26 @@ static inline double bond(const lattice *L, long long n, int a) {
     if (!L->g[a]) return 0.0;
     if (coord(L, n, a) + 1 >= L->dims[a]) return 0.0;
     return (double)L->g[a][n];
+}
+
+/* Neighbour of n along axis a (side 0: forward, 1: backward) and the conductance of the bond between them.
+ * Returns 0 when there is none: a lattice face that does not wrap.  On a wrapping axis the forward entry of
+ * the LAST node is the bond back to the first node (forward-bond convention carried around the ring). */
+static inline int nbr(const lattice *L, long long n, int a, int side, long long *m, double *g) {
+    if (!L->g[a]) return 0;
+    const int c = coord(L, n, a), d = L->dims[a];
+    if (side == 0) {
+        if (c + 1 < d) *m = n + L->stride[a];
+        else if (L->wrap[a]) *m = n - (long long)(d - 1) * L->stride[a];
+        else return 0;
+        *g = (double)L->g[a][n];
+    } else {
+        if (c > 0) *m = n - L->stride[a];
+        else if (L->wrap[a]) *m = n + (long long)(d - 1) * L->stride[a];
+        else return 0;
+        *g = (double)L->g[a][*m];
+    }
+    return 1;
 }
 
 /* ---- S8c steps 2-3: serial breadth-first labelling ------------------------------------------- */
@@ -87,12 +108,7 @@ static int classify(const lattice *L, signed char *cls, pno_info *info) {
                 for (int side = 0; side < 2; ++side) {
                     long long m;
                     double g;
-                    if (side == 0) { g = bond(L, n, a); m = n + L->stride[a]; }
-                    else {
-                        if (coord(L, n, a) == 0) continue;
-                        m = n - L->stride[a];
-                        g = bond(L, m, a);
-                    }
+                    if (!nbr(L, n, a, side, &m, &g)) continue;
                     if (!(g > 0.0)) continue;
                     if (cls[m] == C_INLET) t_in = 1;
                     else if (cls[m] == C_OUTLET) t_out = 1;
@@ -142,10 +158,12 @@ static int assemble(const lattice *L, const signed char *cls, csr *A) {
         if (unk[n] < 0) continue;
         long long cnt = 1;
         A->idx[unk[n]] = n;
-        for (int a = 0; a < 3; ++a) {
-            if (bond(L, n, a) > 0.0 && cls[n + L->stride[a]] == C_SOLVED) ++cnt;
-            if (coord(L, n, a) > 0 && bond(L, n - L->stride[a], a) > 0.0 && cls[n - L->stride[a]] == C_SOLVED) ++cnt;
-        }
+        for (int a = 0; a < 3; ++a)
+            for (int side = 0; side < 2; ++side) {
+                long long mn;
+                double g;
+                if (nbr(L, n, a, side, &mn, &g) && g > 0.0 && cls[mn] == C_SOLVED) ++cnt;
+            }
         A->rowptr[unk[n] + 1] = cnt;
     }
     for (long long u = 0; u < m; ++u) A->rowptr[u + 1] += A->rowptr[u];
@@ -153,7 +171,7 @@ static int assemble(const lattice *L, const signed char *cls, csr *A) {
     A->col = (int *)malloc(sizeof(int) * (size_t)(A->nnz ? A->nnz : 1));
     A->val = (double *)malloc(sizeof(double) * (size_t)(A->nnz ? A->nnz : 1));
     if (!A->col || !A->val) { free(unk); return -1; }
-    /* pass 2: fill, columns ascending (backward z, y, x, diagonal, forward x, y, z) */
+    /* pass 2: fill (backward z, y, x, diagonal, forward x, y, z: columns ascending unless an axis wraps) */
     for (long long n = 0; n < N; ++n) {
         int u = unk[n];
         if (u < 0) continue;
@@ -165,14 +183,7 @@ static int assemble(const lattice *L, const signed char *cls, csr *A) {
                 int a = pass == 0 ? 2 - aa : aa; /* backward: z,y,x ; forward: x,y,z */
                 long long mnode;
                 double g;
-                if (pass == 0) {
-                    if (coord(L, n, a) == 0) continue;
-                    mnode = n - L->stride[a];
-                    g = bond(L, mnode, a);
-                } else {
-                    g = bond(L, n, a);
-                    mnode = n + L->stride[a];
-                }
+                if (!nbr(L, n, a, pass == 0 ? 1 : 0, &mnode, &g)) continue;
                 if (!(g > 0.0)) continue;
                 d += g;
                 if (cls[mnode] == C_INLET) bi += g;
@@ -263,7 +274,8 @@ static void flux(const lattice *L, const double *P, pno_info *info) {
     info->k_eff = info->g_eff * (n_a - 1) / (double)(L->N / n_a);
 }
 
-static int setup(lattice *L, int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int dir) {
+static int setup(lattice *L, int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int dir,
+                 int periodic) {
     if (nx < 1 || ny < 1 || nz < 1 || dir < 0 || dir > 2 || !gx || !gy || (nz > 1 && !gz)) return -1;
     L->nx = nx; L->ny = ny; L->nz = nz; L->dir = dir;
     L->dims[0] = nx; L->dims[1] = ny; L->dims[2] = nz;
@@ -271,10 +283,11 @@ static int setup(lattice *L, int nx, int ny, int nz, const float *gx, const floa
     L->stride[0] = 1; L->stride[1] = nx; L->stride[2] = (long long)nx * ny;
     L->g[0] = gx; L->g[1] = gy; L->g[2] = nz > 1 ? gz : NULL;
     if (L->dims[dir] < 3) return -1;
+    for (int a = 0; a < 3; ++a) L->wrap[a] = periodic && a != dir && L->dims[a] >= 2;
     for (int a = 0; a < 3; ++a) {
         if (!L->g[a]) continue;
         for (long long n = 0; n < L->N; ++n) {
-            if (coord(L, n, a) + 1 >= L->dims[a]) continue;
+            if (coord(L, n, a) + 1 >= L->dims[a] && !L->wrap[a]) continue;
             float g = L->g[a][n];
             if (!(g >= 0.0f) || isinf(g)) return -2;
         }
@@ -284,13 +297,13 @@ static int setup(lattice *L, int nx, int ny, int nz, const float *gx, const floa
 
 /* Whole path.  P_out: N doubles.  classes_out: N bytes or NULL.  max_threads <= 0: all cores.
  * Returns 0 ok / 1 no spanning cluster / 2 max iterations / <0 error. */
-int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction,
+int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction, int periodic,
               double tol, int max_iter, int max_threads, double *P_out, signed char *classes_out, pno_info *info) {
     lattice L;
     pno_info local;
     if (!info) info = &local;
     memset(info, 0, sizeof(*info));
-    int rc = setup(&L, nx, ny, nz, gx, gy, gz, direction);
+    int rc = setup(&L, nx, ny, nz, gx, gy, gz, direction, periodic);
     if (rc) return rc;
 #ifdef _OPENMP
     if (max_threads > 0) omp_set_num_threads(max_threads);
@@ -351,11 +364,11 @@ int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const fl
  * this file's assembled operator, and max |P - pin| over Dirichlet and pinned nodes.  classes_out (N bytes,
  * may be NULL) receives the node classes of the serial labelling. */
 int pno_certificate(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction,
-                    const double *P, double *rel_residual, double *pin_err, signed char *classes_out) {
+                    int periodic, const double *P, double *rel_residual, double *pin_err, signed char *classes_out) {
     lattice L;
     pno_info info;
     memset(&info, 0, sizeof(info));
-    int rc = setup(&L, nx, ny, nz, gx, gy, gz, direction);
+    int rc = setup(&L, nx, ny, nz, gx, gy, gz, direction, periodic);
     if (rc) return rc;
     signed char *cls = classes_out ? classes_out : (signed char *)malloc((size_t)L.N);
     if (!cls || classify(&L, cls, &info)) return -3;

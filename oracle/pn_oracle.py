@@ -10,7 +10,8 @@ What it computes (citations: /root/reference/PAPER.md = `P:<line>`, SURVEY.md 8(
     interior node  ->  G P = b, eq.(3) P:55;
   * boundary conditions, P:57 + S8c readings 1-2: fixed pressure drop along axis `a`, imposed as
     P = 1 on the node plane coord_a = 0 and P = 0 on coord_a = n_a - 1; NO-FLUX on every other face
-    (BASELINE.json north_star / configs[0] bind this; the paper's periodic side faces are "next");
+    (BASELINE.json north_star / configs[0] bind this); `periodic=True` gives the paper's own side condition,
+    lateral axes wrapping around (P:57; S8(f) item 2);
   * isolated / dead-end clusters, S8c step 3 (the paper is silent; north_star mandates it): serial
     breadth-first labelling of interior nodes through open (g > 0) bonds; a component that touches
     both Dirichlet planes is SOLVED, inlet-only is pinned to 1, outlet-only to 0, floating to 0;
@@ -60,8 +61,18 @@ class OracleResult:
 # --------------------------------------------------------------------------------------------------
 # step 1: inputs
 # --------------------------------------------------------------------------------------------------
-def widen(nx, ny, nz, gx, gy, gz):
-    """fp32 -> fp64 exactly; zero the entries that are not bonds (forward neighbour off-lattice)."""
+def wrap_axes(nx, ny, nz, direction, periodic):
+    """Which lattice axes wrap around.  P:57: "periodic boundary conditions in the second direction" -- with
+    `periodic` every LATERAL axis (not the axis of the pressure drop) of length >= 2 wraps: the forward-bond
+    entry of the last node along that axis is then a real bond to the first node.  (Length 1: the wrap bond
+    would join a node to itself and carries nothing.)  Without `periodic`: no-flux faces, nothing wraps."""
+    dims = (nx, ny, nz)
+    return tuple(bool(periodic) and a != direction and dims[a] >= 2 for a in range(3))
+
+
+def widen(nx, ny, nz, gx, gy, gz, wrap=(False, False, False)):
+    """fp32 -> fp64 exactly; zero the entries that are not bonds (forward neighbour off-lattice and the axis
+    does not wrap)."""
     shp = (nz, ny, nx)
     out = []
     for a, g in enumerate((gx, gy, gz)):
@@ -75,7 +86,9 @@ def widen(nx, ny, nz, gx, gy, gz):
             g = g.reshape(shp)
         g64 = g.astype(np.float32).astype(np.float64)
         g64 = g64.copy()
-        if a == 0:
+        if wrap[a]:
+            pass                              # the last entry along a is the bond back to index 0
+        elif a == 0:
             g64[:, :, nx - 1] = 0.0
         elif a == 1:
             g64[:, ny - 1, :] = 0.0
@@ -97,7 +110,7 @@ def _coord_along(nx, ny, nz, direction):
 # --------------------------------------------------------------------------------------------------
 # steps 2-3: node classes by serial breadth-first labelling
 # --------------------------------------------------------------------------------------------------
-def classify(nx, ny, nz, g64, direction):
+def classify(nx, ny, nz, g64, direction, wrap=(False, False, False)):
     """Class of every node (S8c steps 2-3).  Plain serial BFS with an explicit queue.
 
     Edges of the search: interior-interior bonds with g > 0.  `touches_in` / `touches_out` of a
@@ -132,10 +145,17 @@ def classify(nx, ny, nz, g64, direction):
                 g = fl[a][n]
                 if g > 0.0:
                     yield n + stride[a]
+            elif wrap[a]:
+                if fl[a][n] > 0.0:
+                    yield n - (dims[a] - 1) * stride[a]
             if c[a] > 0:
                 m = n - stride[a]
                 g = fl[a][m]
                 if g > 0.0:
+                    yield m
+            elif wrap[a]:
+                m = n + (dims[a] - 1) * stride[a]
+                if fl[a][m] > 0.0:
                     yield m
 
     for seed in range(N):
@@ -174,7 +194,7 @@ def classify(nx, ny, nz, g64, direction):
 # --------------------------------------------------------------------------------------------------
 # dead ends inside the spanning clusters (S8c reading 7, S8(f) item 1)
 # --------------------------------------------------------------------------------------------------
-def dangling_ends(nx, ny, nz, g64, classes):
+def dangling_ends(nx, ny, nz, g64, classes, wrap=(False, False, False)):
     """Boolean mask (nz, ny, nx) of the SOLVED nodes that are dangling (tree-like dead) ends.
 
     Definition (S8c reading 7: "dangling branches inside a spanning cluster have well-defined pressures
@@ -196,10 +216,12 @@ def dangling_ends(nx, ny, nz, g64, classes):
         c = (n % nx, (n // nx) % ny, n // (nx * ny))
         out = []
         for a in range(3):
-            if c[a] + 1 < dims[a] and fl[a][n] > 0.0 and present[n + stride[a]]:
-                out.append(n + stride[a])
-            if c[a] > 0 and fl[a][n - stride[a]] > 0.0 and present[n - stride[a]]:
-                out.append(n - stride[a])
+            up = n + stride[a] if c[a] + 1 < dims[a] else (n - (dims[a] - 1) * stride[a] if wrap[a] else -1)
+            if up >= 0 and fl[a][n] > 0.0 and present[up]:
+                out.append(up)
+            dn = n - stride[a] if c[a] > 0 else (n + (dims[a] - 1) * stride[a] if wrap[a] else -1)
+            if dn >= 0 and fl[a][dn] > 0.0 and present[dn]:
+                out.append(dn)
         return out
 
     stripped = [False] * N
@@ -219,7 +241,7 @@ def dangling_ends(nx, ny, nz, g64, classes):
 # --------------------------------------------------------------------------------------------------
 # step 4: assembled sparse Laplacian over the solved nodes
 # --------------------------------------------------------------------------------------------------
-def assemble(nx, ny, nz, g64, classes):
+def assemble(nx, ny, nz, g64, classes, wrap=(False, False, False)):
     """CSR `A` (fp64) and `b` over SOLVED nodes (S8c step 4).
 
     A_ii = sum of g over ALL open incident bonds (bonds to Dirichlet nodes included),
@@ -242,9 +264,10 @@ def assemble(nx, ny, nz, g64, classes):
     dims = (nx, ny, nz)
     for a in range(3):
         g = g64[a].ravel()
-        has = (coord[a] + 1 < dims[a]) & (g > 0.0)
-        n0 = flat[has]                       # lower end of each open bond
-        n1 = n0 + stride[a]                  # upper end
+        inside = coord[a] + 1 < dims[a]
+        has = (inside | wrap[a]) & (g > 0.0)
+        n0 = flat[has]                       # the end that stores the bond (forward-bond convention)
+        n1 = np.where(inside[has], n0 + stride[a], n0 - (dims[a] - 1) * stride[a])   # other end (wrapped at the face)
         gb = g[has]
         for me, other in ((n0, n1), (n1, n0)):
             mine = solved[me]
@@ -357,18 +380,36 @@ def plane_fluxes(nx, ny, nz, g64, P, direction):
     return np.array([np.sum(gm[c] * (Pm[c] - Pm[c + 1])) for c in range(n_a - 1)])
 
 
-def dissipation(nx, ny, nz, g64, P):
+def dissipation(nx, ny, nz, g64, P, wrap=(False, False, False)):
     """sum over all bonds of g (dP_bond)^2  (= Q * dP at the exact solution; energy identity)."""
     e = 0.0
+    if wrap[0]:
+        e += float(np.sum(g64[0][:, :, -1] * (P[:, :, 0] - P[:, :, -1]) ** 2))
+    if wrap[1]:
+        e += float(np.sum(g64[1][:, -1, :] * (P[:, 0, :] - P[:, -1, :]) ** 2))
+    if wrap[2]:
+        e += float(np.sum(g64[2][-1, :, :] * (P[0, :, :] - P[-1, :, :]) ** 2))
     e += float(np.sum(g64[0][:, :, :-1] * (P[:, :, 1:] - P[:, :, :-1]) ** 2))
     e += float(np.sum(g64[1][:, :-1, :] * (P[:, 1:, :] - P[:, :-1, :]) ** 2))
     e += float(np.sum(g64[2][:-1, :, :] * (P[1:, :, :] - P[:-1, :, :]) ** 2))
     return e
 
 
-def kirchhoff_residual(nx, ny, nz, g64, P):
+def kirchhoff_residual(nx, ny, nz, g64, P, wrap=(False, False, False)):
     """Net current into every node, sum_j g_ij (P_j - P_i), on the whole lattice."""
     r = np.zeros((nz, ny, nx))
+    if wrap[0]:
+        f = g64[0][:, :, -1] * (P[:, :, 0] - P[:, :, -1])
+        r[:, :, -1] += f
+        r[:, :, 0] -= f
+    if wrap[1]:
+        f = g64[1][:, -1, :] * (P[:, 0, :] - P[:, -1, :])
+        r[:, -1, :] += f
+        r[:, 0, :] -= f
+    if wrap[2]:
+        f = g64[2][-1, :, :] * (P[0, :, :] - P[-1, :, :])
+        r[-1, :, :] += f
+        r[0, :, :] -= f
     fx = g64[0][:, :, :-1] * (P[:, :, 1:] - P[:, :, :-1])
     r[:, :, :-1] += fx
     r[:, :, 1:] -= fx
@@ -384,17 +425,19 @@ def kirchhoff_residual(nx, ny, nz, g64, P):
 # --------------------------------------------------------------------------------------------------
 # the whole path
 # --------------------------------------------------------------------------------------------------
-def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, dense=False):
-    """Pressures on all nodes + effective conductance (S8c steps 1-8)."""
-    g64 = widen(nx, ny, nz, gx, gy, gz)
-    classes = classify(nx, ny, nz, g64, direction)
+def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, dense=False, periodic=False):
+    """Pressures on all nodes + effective conductance (S8c steps 1-8).  `periodic`: lateral faces wrap (the
+    paper's own side condition) instead of the default no-flux faces (north_star)."""
+    wrap = wrap_axes(nx, ny, nz, direction, periodic)
+    g64 = widen(nx, ny, nz, gx, gy, gz, wrap)
+    classes = classify(nx, ny, nz, g64, direction, wrap)
     P = pin_values(classes)
     counts = [int(np.sum(classes == c)) for c in (SOLVED, INLET_ONLY, OUTLET_ONLY, FLOATING)]
     if counts[0] == 0:
         q_in, q_out, g_eff, k_eff = flux(nx, ny, nz, g64, P, direction)
         return OracleResult(P, classes, q_in, q_out, g_eff, k_eff, 0, 0, 0.0, *counts,
                             "no_spanning_cluster")
-    A, b, diag, idx = assemble(nx, ny, nz, g64, classes)
+    A, b, diag, idx = assemble(nx, ny, nz, g64, classes, wrap)
     if dense:
         x = np.linalg.solve(A.toarray(), b)
         it, restarts = 0, 0
@@ -408,14 +451,15 @@ def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, dense
                         status)
 
 
-def residual_certificate(nx, ny, nz, gx, gy, gz, P, direction, classes=None):
+def residual_certificate(nx, ny, nz, gx, gy, gz, P, direction, classes=None, periodic=False):
     """Independent check of ANY pressure field: ||b - A P_S||2 / ||b||2 with the oracle's own
     assembled operator (S8c last pin row: one CPU SpMV, usable at sizes where a second solve is
     too slow).  Returns (rel_residual, max |P - pin| over pinned and Dirichlet nodes)."""
-    g64 = widen(nx, ny, nz, gx, gy, gz)
+    wrap = wrap_axes(nx, ny, nz, direction, periodic)
+    g64 = widen(nx, ny, nz, gx, gy, gz, wrap)
     if classes is None:
-        classes = classify(nx, ny, nz, g64, direction)
-    A, b, diag, idx = assemble(nx, ny, nz, g64, classes)
+        classes = classify(nx, ny, nz, g64, direction, wrap)
+    A, b, diag, idx = assemble(nx, ny, nz, g64, classes, wrap)
     P = np.asarray(P, dtype=np.float64).reshape(nz, ny, nx)
     pins = pin_values(classes)
     not_solved = classes != SOLVED

@@ -97,3 +97,33 @@ def test_c_oracle_no_spanning_cluster_and_errors():
     net = inputs.cfg1_iid_2d(32, 32, seed=0)
     r = crun(net, 0, tol=1e-13, max_iter=5)
     assert r.status == "max_iters" and r.iterations == 5 and r.rel_residual > 1e-13
+
+
+# ---------------------------------------------------------------- periodic lateral faces ---
+def test_c_oracle_periodic_hand_worked_example():
+    """tests/golden/worked_3x2_periodic.txt: 55/141, 57/141, 338/141."""
+    gx = np.array([[[1, 2, 99], [3, 4, 99]]], dtype=np.float32)
+    gy = np.array([[[77, 5, 77], [88, 7, 88]]], dtype=np.float32)
+    r = c_oracle.solve(3, 2, 1, gx, gy, None, 0, 1e-15, periodic=True)
+    assert r.P[0, 0, 1] == pytest.approx(55 / 141, abs=1e-14)
+    assert r.P[0, 1, 1] == pytest.approx(57 / 141, abs=1e-14)
+    assert r.g_eff == pytest.approx(338 / 141, rel=1e-13)
+
+
+@pytest.mark.parametrize("maker,direction", [
+    (lambda: inputs.cfg1_iid_2d(40, 33, seed=0), 0),
+    (lambda: inputs.cfg3_percolation_3d(20, 18, 16, seed=2, p=0.35), 0),
+    (lambda: inputs.cfg4_fbm_cut_3d(20, 20, 20, seed=3), 1),
+    (lambda: inputs.iid_diluted(9, 2, 7, seed=5, p=0.8), 2),
+])
+def test_c_oracle_periodic_matches_python_oracle(maker, direction):
+    net = maker()
+    a = po.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13, periodic=True)
+    b = c_oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13, periodic=True)
+    assert np.array_equal(a.classes, b.classes)
+    assert np.max(np.abs(a.P - b.P)) < 1e-11
+    assert b.g_eff == pytest.approx(a.g_eff, rel=1e-11)
+    rel, pin = c_oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, a.P, direction, periodic=True)
+    assert rel <= 1e-13 and pin == 0.0
+    rel0, _ = c_oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, a.P, direction)
+    assert rel0 > 1e-6          # the no-flux operator rejects the periodic solution

@@ -112,7 +112,7 @@ def test_hand_worked_3x2_example():
 
 
 # ---------------------------------------------------------------- dense cross-check ----------------
-def brute_force_dense(net, direction):
+def brute_force_dense(net, direction, periodic=False):
     """Independent statement of the problem: full N x N graph Laplacian built bond by bond in Python
     loops, Dirichlet rows replaced by identity, nodes with no path to a Dirichlet plane... are
     handled by least-norm-free elimination: we solve only on nodes connected to a Dirichlet node."""
@@ -126,10 +126,15 @@ def brute_force_dense(net, direction):
         n = i + nx * (j + ny * k)
         c = (i, j, k)
         for a in range(3):
-            if gs[a] is None or c[a] + 1 >= dims[a]:
+            if gs[a] is None:
+                continue
+            if c[a] + 1 < dims[a]:
+                m = n + stride[a]
+            elif periodic and a != direction and dims[a] >= 2:
+                m = n - (dims[a] - 1) * stride[a]          # lateral faces wrap
+            else:
                 continue
             g = float(gs[a][k, j, i])
-            m = n + stride[a]
             L[n, n] += g
             L[m, m] += g
             L[n, m] -= g
@@ -387,15 +392,23 @@ def test_residual_certificate_detects_a_wrong_field():
 
 
 # ---------------------------------------------------------------- dangling ends (S8c reading 7) ---
-def _open_nbrs(nx, ny, nz, g64, n):
+def _open_nbrs(nx, ny, nz, g64, n, wrap=(False, False, False)):
     """Open-bond neighbours of node n, written independently of the oracle (coordinate loops)."""
     i, j, k = n % nx, (n // nx) % ny, n // (nx * ny)
     out = []
     for (di, dj, dk) in ((1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)):
         a, b, c = i + di, j + dj, k + dk
-        if not (0 <= a < nx and 0 <= b < ny and 0 <= c < nz):
-            continue
         arr = g64[0] if di else (g64[1] if dj else g64[2])
+        if not (0 <= a < nx and 0 <= b < ny and 0 <= c < nz):
+            ax = 0 if di else (1 if dj else 2)
+            if not wrap[ax]:
+                continue
+            a, b, c = a % nx, b % ny, c % nz
+            # the wrap bond is stored at the LAST node along the axis
+            g = arr[max(k, c), max(j, b), max(i, a)]
+            if g > 0.0:
+                out.append(a + nx * (b + ny * c))
+            continue
         g = arr[min(k, c), min(j, b), min(i, a)]        # the forward bond lives on the lower-index end
         if g > 0.0:
             out.append(a + nx * (b + ny * c))
@@ -404,19 +417,20 @@ def _open_nbrs(nx, ny, nz, g64, n):
 
 @pytest.mark.parametrize("shape,direction,p,seed", [((5, 4, 1), 0, 0.7, s) for s in range(6)] +
                          [((4, 5, 1), 1, 0.75, s) for s in range(4)] + [((4, 3, 3), 0, 0.6, s) for s in range(6)])
-def test_dangling_ends_equal_complement_of_bruteforce_2core(shape, direction, p, seed):
+def test_dangling_ends_equal_complement_of_bruteforce_2core(shape, direction, p, seed, periodic=False):
     """The nodes left after stripping are the 2-core (Dirichlet nodes kept): the UNION of all node subsets in
     which every member keeps >= 2 open neighbours inside (subset + Dirichlet planes).  Enumerated outright."""
     nx, ny, nz = shape
     net = inputs.iid_diluted(nx, ny, nz, seed=100 + seed, p=p)
-    g64 = po.widen(nx, ny, nz, net.gx, net.gy, net.gz)
-    cls = po.classify(nx, ny, nz, g64, direction)
-    mask = po.dangling_ends(nx, ny, nz, g64, cls)
+    wrap = po.wrap_axes(nx, ny, nz, direction, periodic)
+    g64 = po.widen(nx, ny, nz, net.gx, net.gy, net.gz, wrap)
+    cls = po.classify(nx, ny, nz, g64, direction, wrap)
+    mask = po.dangling_ends(nx, ny, nz, g64, cls, wrap)
     flat = cls.ravel()
     solved = [n for n in range(nx * ny * nz) if flat[n] == po.SOLVED]
     assert len(solved) <= 18
     dirichlet = {n for n in range(nx * ny * nz) if flat[n] in (po.INLET, po.OUTLET)}
-    nbrs = {n: _open_nbrs(nx, ny, nz, g64, n) for n in solved}
+    nbrs = {n: _open_nbrs(nx, ny, nz, g64, n, wrap) for n in solved}
     core = set()
     for bits in range(1 << len(solved)):
         sub = {solved[t] for t in range(len(solved)) if bits >> t & 1}
@@ -473,3 +487,96 @@ def test_dangling_ends_carry_no_current(direction):
     assert worst < 1e-11
     # and some bond that is NOT at a dangling node does carry current
     assert max(float(np.max(np.abs(c))) for c in cur) > 1e-3
+
+
+# ---------------------------------------------------------------- periodic lateral faces ---
+def test_periodic_hand_worked_3x2_example():
+    """tests/golden/worked_3x2_periodic.txt: the wrap bond doubles the a-b connection; 55/141, 57/141, 338/141."""
+    vals = {}
+    for line in open(os.path.join(GOLDEN, "worked_3x2_periodic.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        vals[k] = Fraction(v)
+    gx = np.array([[[1, 2, 99], [3, 4, 99]]], dtype=np.float32)
+    gy = np.array([[[77, 5, 77], [88, 7, 88]]], dtype=np.float32)   # 77/88: bonds inside the Dirichlet columns
+    res = po.solve(3, 2, 1, gx, gy, None, 0, 1e-15, periodic=True)
+    assert res.P[0, 0, 1] == pytest.approx(float(vals["Pa"]), abs=1e-14)
+    assert res.P[0, 1, 1] == pytest.approx(float(vals["Pb"]), abs=1e-14)
+    assert res.g_eff == pytest.approx(float(vals["G_eff"]), rel=1e-13)
+    assert res.q_in == pytest.approx(res.q_out, rel=1e-13)
+    # without the flag the wrap entry is not a bond: the no-flux golden values (27/71, 29/71)
+    res0 = po.solve(3, 2, 1, gx, gy, None, 0, 1e-15)
+    assert res0.P[0, 0, 1] == pytest.approx(27 / 71, abs=1e-14)
+
+
+@pytest.mark.parametrize("shape,direction", [((9, 6, 5), 0), ((9, 6, 5), 1), ((9, 6, 5), 2), ((7, 4, 1), 0), ((7, 4, 1), 1)])
+def test_periodic_uniform_closed_form(shape, direction):
+    nx, ny, nz = shape
+    net = inputs.uniform(nx, ny, nz, 0.37)
+    res = run(net, direction, periodic=True)
+    n_a = shape[direction]
+    coord = po._coord_along(nx, ny, nz, direction)[0]
+    assert np.max(np.abs(res.P - (1.0 - coord / (n_a - 1)))) < 1e-12
+    assert res.g_eff == pytest.approx(float(np.float32(0.37)) * (nx * ny * nz // n_a) / (n_a - 1), rel=1e-12)
+
+
+@pytest.mark.parametrize("shape,p,seed,direction", [
+    ((6, 5, 1), 1.0, 1, 0), ((6, 5, 1), 0.7, 2, 1), ((5, 4, 3), 1.0, 3, 2), ((5, 4, 3), 0.6, 4, 0),
+    ((4, 5, 4), 0.5, 5, 1), ((8, 8, 1), 0.6, 6, 0), ((7, 2, 5), 0.7, 8, 2), ((5, 2, 1), 0.9, 9, 0)])
+def test_periodic_against_dense_lapack_on_bruteforce_laplacian(shape, p, seed, direction):
+    """Same independent dense statement as the no-flux case, with the wrap bonds added bond by bond (lengths 2 and
+    1 along a lateral axis included: a doubled bond, resp. no wrap bond at all)."""
+    net = inputs.iid_diluted(*shape, seed=seed, p=p)
+    res = run(net, direction, periodic=True)
+    Pd, connected = brute_force_dense(net, direction, periodic=True)
+    defined = res.classes != po.FLOATING
+    assert np.max(np.abs(res.P[defined] - Pd[defined])) < 1e-11
+    interior = set(np.flatnonzero((res.classes.ravel() != po.INLET) & (res.classes.ravel() != po.OUTLET)).tolist())
+    assert set(np.flatnonzero(res.classes.ravel() == po.FLOATING).tolist()) == interior - connected
+    # and the flag matters on these inputs (the wrap bonds carry current)
+    if p == 1.0:
+        assert abs(run(net, direction).g_eff - res.g_eff) > 1e-6 * res.g_eff
+
+
+@pytest.mark.parametrize("direction,axis,shift", [(0, 1, 3), (0, 2, 2), (2, 0, 5), (1, 2, 1)])
+def test_periodic_translation_invariance(direction, axis, shift):
+    """A cyclic shift of the network along a lateral axis shifts the solution and leaves G_eff alone -- true for
+    periodic faces only (with no-flux faces the shifted network is a different problem)."""
+    net = inputs.iid_diluted(8, 7, 6, seed=12, p=0.8)
+    ax = 2 - axis                                    # numpy axis of lattice axis `axis`
+    roll = lambda a: np.roll(a, shift, axis=ax)
+    a = run(net, direction, periodic=True)
+    b = po.solve(net.nx, net.ny, net.nz, roll(net.gx), roll(net.gy), roll(net.gz), direction, 1e-13, periodic=True)
+    assert np.max(np.abs(roll(a.P) - b.P)) < 1e-11
+    assert b.g_eff == pytest.approx(a.g_eff, rel=1e-11)
+    assert np.array_equal(roll(a.classes), b.classes)
+    c = run(net, direction)
+    d = po.solve(net.nx, net.ny, net.nz, roll(net.gx), roll(net.gy), roll(net.gz), direction, 1e-13)
+    assert abs(c.g_eff - d.g_eff) > 1e-6 * c.g_eff
+
+
+@pytest.mark.parametrize("maker,direction", [
+    (lambda: inputs.cfg3_percolation_3d(12, 11, 10, seed=2, p=0.45), 0),
+    (lambda: inputs.cfg4_fbm_cut_3d(12, 12, 12, seed=3), 1),
+    (lambda: inputs.iid_diluted(20, 17, 1, seed=3, p=0.7), 1)])
+def test_periodic_conservation_invariants(maker, direction):
+    net = maker()
+    res = run(net, direction, periodic=True)
+    wrap = po.wrap_axes(net.nx, net.ny, net.nz, direction, True)
+    g64 = po.widen(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, wrap)
+    kr = po.kirchhoff_residual(net.nx, net.ny, net.nz, g64, res.P, wrap)
+    assert np.max(np.abs(kr[res.classes == po.SOLVED])) < 1e-11 * max(res.q_in, 1.0)
+    pf = po.plane_fluxes(net.nx, net.ny, net.nz, g64, res.P, direction)
+    assert np.max(np.abs(pf - pf[0])) < 1e-11 * max(abs(pf[0]), 1.0)
+    assert po.dissipation(net.nx, net.ny, net.nz, g64, res.P, wrap) == pytest.approx(res.g_eff, rel=1e-10, abs=1e-13)
+    rel, pin_err = po.residual_certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, res.P, direction, periodic=True)
+    assert rel <= 1e-13 and pin_err == 0.0
+    # the certificate of the OTHER boundary condition rejects this field
+    rel0, _ = po.residual_certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, res.P, direction)
+    assert rel0 > 1e-6
+
+
+@pytest.mark.parametrize("shape,direction,p,seed", [((5, 4, 1), 0, 0.6, s) for s in range(4)] + [((4, 3, 3), 0, 0.5, s) for s in range(4)])
+def test_periodic_dangling_ends_bruteforce_2core(shape, direction, p, seed):
+    test_dangling_ends_equal_complement_of_bruteforce_2core(shape, direction, p, seed, periodic=True)
