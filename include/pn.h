@@ -95,6 +95,12 @@ enum {
                                + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused)      */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
+    PN_OPT_LATERAL = 8,     /* lateral (side) faces: 0 (default) = no-flux (north_star, configs[0]); 1 = periodic,
+                               the paper's own condition ("periodic boundary conditions in the second
+                               direction"; S8(f) item 2): every axis other than the solve axis wraps around, and
+                               the forward entry of the LAST node along such an axis is the bond back to the
+                               first node (validated at pn_solve: PN_ERR_VALUE).  An axis of one node does
+                               not wrap                                                             */
     PN_OPT_PEEL = 7         /* dead-end peeling: solved nodes left with one open bond carry no current
                                (S8(c) reading 7, S8(f) item 1); they are removed from the system,
                                recursively, and take the pressure of the node they hang from after the

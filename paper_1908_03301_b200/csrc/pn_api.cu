@@ -33,7 +33,8 @@ struct pn_ctx {
     bool have_g, have_solution, ever_solved;
     int last_dir_user;
     // options
-    int max_iters, chunk, x0_linear, skip_label, variant, profile, peel;
+    int max_iters, chunk, x0_linear, skip_label, variant, profile, peel, lateral;
+    int base_closed;            // some in-lattice (non-wrap) bond is closed: from S0's validation
     cudaEvent_t* pev;           // event pool for PN_OPT_PROFILE (2*chunk+1), created on demand
     int pev_n;
     double delta;
@@ -53,7 +54,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct layout {
     pn_geom g;
-    size_t off_raw[3], off_gs[3], off_w[3], off_s, off_x64, off_r, off_p, off_p2, off_q, off_xh, off_r2, off_q2, off_cls, off_slots,
+    size_t off_raw[3], off_gs[3], off_w[3], off_gsw[3], off_ww[3], off_s, off_x64, off_r, off_p, off_p2, off_q, off_xh, off_r2, off_q2, off_cls, off_slots,
         off_state, total;
     size_t halo;                // elements in one halo plane
 };
@@ -70,6 +71,7 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     g.npad = g.plane * g.nz;
     g.n = (long long)nx * ny * nz;
     g.dir = 0; g.n_a = nx; g.stride_a = 1;
+    g.wrap[0] = g.wrap[1] = g.wrap[2] = 0;
     if (g.npad + 2 * g.plane >= (1ll << 31)) return false;
     L->halo = (size_t)g.plane;
     const size_t vec = (size_t)g.npad + 2 * L->halo;   // elements of a padded array with its two halo planes
@@ -78,6 +80,8 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     for (int b = 0; b < 3; ++b) L->off_raw[b] = take((size_t)g.n * 4);
     for (int b = 0; b < 3; ++b) L->off_gs[b] = take(vec * 4);
     for (int b = 0; b < 3; ++b) L->off_w[b] = take(vec * 4);
+    for (int b = 0; b < 3; ++b) L->off_gsw[b] = take((size_t)pn_face_count(g, b) * 4);
+    for (int b = 0; b < 3; ++b) L->off_ww[b] = take((size_t)pn_face_count(g, b) * 4);
     L->off_s = take(vec * 4);
     L->off_x64 = take(vec * 8);
     L->off_r = take(vec * 4);
@@ -159,6 +163,8 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
         ctx->raw_store[b] = (float*)(ctx->ws + L.off_raw[b]);
         P.gs[b] = (float*)(ctx->ws + L.off_gs[b]) + h;
         P.w[b] = (float*)(ctx->ws + L.off_w[b]) + h;
+        P.gsw[b] = (float*)(ctx->ws + L.off_gsw[b]);
+        P.ww[b] = (float*)(ctx->ws + L.off_ww[b]);
     }
     P.s = (float*)(ctx->ws + L.off_s) + h;
     P.x64 = (double*)(ctx->ws + L.off_x64) + h;
@@ -212,6 +218,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
         case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
+        case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
@@ -261,6 +268,7 @@ int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const flo
     CK(cudaMemcpyAsync(ctx->h_state, ctx->P.st, sizeof(pn_state), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     if (ctx->h_state->bad_value) return PN_ERR_VALUE;
+    ctx->base_closed = ctx->h_state->any_closed;
     ctx->have_g = true;
     return PN_OK;
 }
@@ -287,6 +295,10 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     g.dir = (ctx->is2d && direction == 1) ? 2 : direction;
     g.n_a = ulen[direction];
     g.stride_a = g.dir == 0 ? 1 : (g.dir == 1 ? g.px : g.plane);
+    // periodic lateral faces: every internal axis but the solve axis wraps, if it has >= 2 nodes
+    const int idims[3] = {g.nx, g.ny, g.nz};
+    bool any_wrap = false;
+    for (int b = 0; b < 3; ++b) { g.wrap[b] = (ctx->lateral == 1 && b != g.dir && idims[b] >= 2) ? 1 : 0; any_wrap |= g.wrap[b] != 0; }
     const pn_ptrs& P = ctx->P;
     cudaStream_t s = ctx->stream;
     int nl = 0;
@@ -299,14 +311,24 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     const int scheme = pn_resolve_variant(g, ctx->variant);
     const int fused = scheme == 3;
-    const bool do_label = !ctx->skip_label && ctx->h_state->any_closed;
+    int any_closed = ctx->base_closed;
+    if (any_wrap) {
+        // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
+        CK(cudaMemsetAsync(&P.st->bad_value, 0, 2 * sizeof(int), s));
+        CK(pn_launch_wrap_copy(g, P, s, &nl));
+        rc = read_state(ctx);
+        if (rc) return rc;
+        if (ctx->h_state->bad_value) { ctx->launches += nl; return PN_ERR_VALUE; }
+        any_closed |= ctx->h_state->any_closed;
+    }
+    const bool do_label = !ctx->skip_label && any_closed;
     const bool do_peel = do_label && ctx->peel;
     const int x0_mode = (ctx->x0_linear == 2 && !ctx->ever_solved) ? 1 : ctx->x0_linear;   // nothing to warm-start from yet
     CK(pn_launch_label(g, P, do_label, do_peel, x0_mode, s, &nl));
     if (do_peel && ctx->peel == 2) {
         // automatic: keep the peeling only if it removes at least PN_PEEL_MIN_FRACTION of the unknowns.  Peeled nodes are
         // still streamed (structured storage), so the gain is fewer iterations only; measured on B200:
-        // 52 % peeled -> -28 % iterations (CFG3), 3.8 % peeled -> +1.8 % (CFG4: within the noise of the iteration count)
+        // 52 % peeled -> -28 % iterations (CFG3), 3.8 % peeled -> +1.8 % (CFG4: no gain)
         rc = read_state(ctx);
         if (rc) return rc;
         if ((double)ctx->h_state->n_peeled < PN_PEEL_MIN_FRACTION * (double)ctx->h_state->count[0]) {

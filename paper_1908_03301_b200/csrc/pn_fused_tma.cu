@@ -66,35 +66,6 @@ struct alignas(64) pn_fmaps {
     CUtensorMap wx_main, wx_slv, wy, wz;
 };
 
-// Last-block epilogue: alpha_t, the predicted beta_{t+1}, bookkeeping and the triggers the host polls for.
-__device__ __forceinline__ void finish_F(pn_state* st, double rr, double pq, double rq, double qq) {
-    st->rr_old = st->rr;
-    st->rr = rr;
-    st->pq = pq;
-    const int it = st->iters + 1;
-    st->iters = it;
-    double rr_max = st->rr_max;
-    if (rr > rr_max) { rr_max = rr; st->rr_max = rr_max; }
-    int flag = PN_FLAG_RUN;
-    double alpha = 0.0, beta = 0.0;
-    if (!(rr >= 0.0) || isinf(rr)) flag = PN_FLAG_BREAKDOWN;
-    else if (rr == 0.0) flag = PN_FLAG_CONVERGED;
-    else if (!(pq > 0.0) || isinf(pq)) flag = PN_FLAG_BREAKDOWN;
-    else {
-        alpha = rr / pq;
-        const double rr_next = rr - 2.0 * alpha * rq + alpha * alpha * qq;   // ||r_t - alpha_t q_t||^2
-        if (rr <= st->rr_target) flag = PN_FLAG_CONVERGED;
-        else if (rr < st->delta2 * rr_max) flag = PN_FLAG_UPDATE;
-        else if (it >= st->max_iters) flag = PN_FLAG_BUDGET;
-        else if (!(rr_next > 0.0) || isinf(rr_next)) flag = PN_FLAG_UPDATE;   // prediction lost: replace the residual
-        else beta = rr_next / rr;
-    }
-    st->alpha = alpha;      // alpha_t: next kernel's residual and solution updates
-    st->alpha_x = alpha;    // ... and what k_flush applies to the pending direction p_t
-    st->beta = beta;
-    st->flag = flag;
-}
-
 template <class C>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
 k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz) {
@@ -297,7 +268,11 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     a_qq = pn_block_sum(a_qq, red);
     const double v4[4] = {a_rr, a_pq, a_rq, a_qq};
     if (pn_grid_sum<4>(v4, P.slots, &st->ticket, red, red + 32)) {
-        if (threadIdx.x == 0) finish_F(st, red[32], red[33], red[34], red[35]);
+        if (threadIdx.x == 0) {
+            if (g.wrap[0] | g.wrap[1] | g.wrap[2]) {   // periodic faces: k_wrap_fix adds the wrap bonds' part and finishes
+                st->part[0] = red[32]; st->part[1] = red[33]; st->part[2] = red[34]; st->part[3] = red[35];
+            } else pn_finish_F(st, red[32], red[33], red[34], red[35]);
+        }
     }
 }
 

@@ -32,14 +32,6 @@ __device__ __forceinline__ float4 fma4(float a, const float4& x, const float4& y
     return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
 }
 
-// Last-block epilogue of kernel A: alpha = rr / (p.Ap); breakdown guards.
-__device__ __forceinline__ void finish_A(pn_state* st, double pq) {
-    st->pq = pq;
-    if (st->rr == 0.0) st->flag = PN_FLAG_CONVERGED;
-    else if (!(pq > 0.0) || isinf(pq)) st->flag = PN_FLAG_BREAKDOWN;
-    else st->alpha = st->rr / pq;
-}
-
 // Last-block epilogue of kernel B: beta, bookkeeping, and the triggers the host polls for.
 __device__ __forceinline__ void finish_B(pn_state* st, double rr_new) {
     const double rr_old = st->rr;
@@ -58,7 +50,7 @@ __device__ __forceinline__ void finish_B(pn_state* st, double rr_new) {
 }
 
 // ---- kernel A, reference variant: one thread per 4 consecutive nodes, neighbours through L1/L2 ---
-__global__ void __launch_bounds__(TPB) k_stencil_simple(int nvec, int px, int plane, pn_ptrs P, float* p0, float* p1) {
+__global__ void __launch_bounds__(TPB) k_stencil_simple(int nvec, int px, int plane, pn_ptrs P, float* p0, float* p1, int defer) {
     pn_state* st = P.st;
     if (st->flag != PN_FLAG_RUN) return;
     __shared__ double sm[32];
@@ -99,7 +91,10 @@ __global__ void __launch_bounds__(TPB) k_stencil_simple(int nvec, int px, int pl
     acc = pn_block_sum(acc, sm);
     const double v1[1] = {acc};
     if (pn_grid_sum<1>(v1, P.slots, &st->ticket, sm, tot)) {
-        if (threadIdx.x == 0) finish_A(st, tot[0]);
+        if (threadIdx.x == 0) {
+            if (defer) st->part[0] = tot[0];   // periodic faces: k_wrap_fix finishes
+            else pn_finish_A(st, tot[0]);
+        }
     }
 }
 
@@ -167,18 +162,20 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     pn_fused_plan* fplan = nullptr;
     if (scheme == 2 && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) return cudaErrorNotSupported;
     if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
+    const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];   // periodic lateral faces: k_wrap_fix finishes kernel A
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);
     for (int it = 0; it < iterations && e == cudaSuccess; ++it) {
         if (scheme == 3) e = pn_launch_cg_fused(fplan, g, P, st);
         else if (scheme == 2) e = pn_launch_stencil_tma(plan, g, P, st);
-        else k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2);
+        else k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2, wrap ? 1 : 0);
+        if (wrap && e == cudaSuccess) e = pn_launch_wrap_fix(g, P, scheme == 3, st);
         if (ev) cudaEventRecord(ev[2 * it + 1], st);
         if (scheme != 3) k_update<<<nb, TPB, 0, st>>>(nvec, P);
         if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
     pn_tma_plan_free(plan);
     pn_fused_plan_free(fplan);
-    *launches += (scheme == 3 ? 1 : 2) * iterations;
+    *launches += ((scheme == 3 ? 1 : 2) + (wrap ? 1 : 0)) * iterations;
     return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -30,7 +30,22 @@ struct pn_geom {
     int dir;                    // INTERNAL solve axis 0/1/2
     int n_a;                    // lattice length along dir
     long long stride_a;         // element stride along dir (1, px, plane)
+    int wrap[3];                // INTERNAL axis wraps around (periodic lateral faces); never `dir`, never a length-1 axis
 };
+
+// ---- periodic lateral faces: the wrap bonds live in small FACE arrays, not in the lattice-shaped ones ----
+// (the flat-index stencil of the lattice arrays knows nothing about them; k_wrap_fix adds their part of q).
+// Face of axis b = the nodes with coordinate 0 along b, indexed  b=0: j + ny*k,  b=1: i + px*k,  b=2: i + px*j.
+// Entry f of a face array = the bond between the node at coordinate dims[b]-1 ("hi") and the node at 0 ("lo").
+__host__ __device__ inline long long pn_face_count(const pn_geom& g, int b) {
+    return b == 0 ? (long long)g.ny * g.nz : (b == 1 ? (long long)g.px * g.nz : g.plane);
+}
+__host__ __device__ inline long long pn_face_index(const pn_geom& g, int b, int i, int j, int k) {
+    return b == 0 ? j + (long long)g.ny * k : (b == 1 ? i + (long long)g.px * k : i + (long long)g.px * j);
+}
+__host__ __device__ inline long long pn_wrap_span(const pn_geom& g, int b) {   // flat distance lo -> hi
+    return b == 0 ? (long long)(g.nx - 1) : (b == 1 ? (long long)(g.ny - 1) * g.px : (long long)(g.nz - 1) * g.plane);
+}
 
 // Device-resident scalars of the inner iteration (S8(a) S6: alpha, beta never leave the device).
 struct pn_state {
@@ -43,6 +58,7 @@ struct pn_state {
     double rr_max;              // largest rr since the last fp64 residual replacement
     double rr_target;           // proxy exit threshold on rr (set by the host from tol)
     double delta2;              // reliable-update threshold squared
+    double part[4];             // periodic faces: the main kernel's sums, finished by k_wrap_fix (rr, pq, rq, qq | pq)
     double acc[4];              // results of the fp64 reductions (residual norms, b norm, flux)
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
     unsigned long long n_peeled;// solved nodes removed from the system as dangling ends (back-filled after the solve)
@@ -55,6 +71,44 @@ struct pn_state {
 };
 
 enum { PN_FLAG_RUN = 0, PN_FLAG_CONVERGED = 1, PN_FLAG_UPDATE = 2, PN_FLAG_BREAKDOWN = 3, PN_FLAG_BUDGET = 4 };
+
+// ---- last-block epilogues of the inner iteration (shared by the main kernels and k_wrap_fix) ----
+// Last-block epilogue of kernel A: alpha = rr / (p.Ap); breakdown guards.
+__device__ __forceinline__ void pn_finish_A(pn_state* st, double pq) {
+    st->pq = pq;
+    if (st->rr == 0.0) st->flag = PN_FLAG_CONVERGED;
+    else if (!(pq > 0.0) || isinf(pq)) st->flag = PN_FLAG_BREAKDOWN;
+    else st->alpha = st->rr / pq;
+}
+
+// Last-block epilogue: alpha_t, the predicted beta_{t+1}, bookkeeping and the triggers the host polls for.
+__device__ __forceinline__ void pn_finish_F(pn_state* st, double rr, double pq, double rq, double qq) {
+    st->rr_old = st->rr;
+    st->rr = rr;
+    st->pq = pq;
+    const int it = st->iters + 1;
+    st->iters = it;
+    double rr_max = st->rr_max;
+    if (rr > rr_max) { rr_max = rr; st->rr_max = rr_max; }
+    int flag = PN_FLAG_RUN;
+    double alpha = 0.0, beta = 0.0;
+    if (!(rr >= 0.0) || isinf(rr)) flag = PN_FLAG_BREAKDOWN;
+    else if (rr == 0.0) flag = PN_FLAG_CONVERGED;
+    else if (!(pq > 0.0) || isinf(pq)) flag = PN_FLAG_BREAKDOWN;
+    else {
+        alpha = rr / pq;
+        const double rr_next = rr - 2.0 * alpha * rq + alpha * alpha * qq;   // ||r_t - alpha_t q_t||^2
+        if (rr <= st->rr_target) flag = PN_FLAG_CONVERGED;
+        else if (rr < st->delta2 * rr_max) flag = PN_FLAG_UPDATE;
+        else if (it >= st->max_iters) flag = PN_FLAG_BUDGET;
+        else if (!(rr_next > 0.0) || isinf(rr_next)) flag = PN_FLAG_UPDATE;   // prediction lost: replace the residual
+        else beta = rr_next / rr;
+    }
+    st->alpha = alpha;      // alpha_t: next kernel's residual and solution updates
+    st->alpha_x = alpha;    // ... and what k_flush applies to the pending direction p_t
+    st->beta = beta;
+    st->flag = flag;
+}
 
 // ---- reductions: warp shuffle -> block -> per-block slot -> last block sums slots in fixed order ----
 __device__ __forceinline__ double pn_warp_sum(double v) {
@@ -112,6 +166,8 @@ struct pn_ptrs {
     const float* raw[3];        // user-layout copies of the conductances (raw[1] == nullptr for 2D)
     float* gs[3];               // solve copy: pruned, off-lattice entries zeroed (padded layout)
     float* w[3];                // symmetric-Jacobi-scaled bond weights of the fp32 inner system
+    float* gsw[3];              // face arrays: solve copy of the wrap bonds (periodic lateral faces)
+    float* ww[3];               // face arrays: their scaled weights
     float* s;                   // s_i = 1/sqrt(diag_i) on solved nodes, 0 elsewhere
     double* x64;                // pressures (fp64), all nodes
     float *r, *p, *p2, *q, *xh; // fp32 CG vectors of the scaled system (p, p2: double-buffered search direction)
@@ -148,6 +204,10 @@ struct pn_fused_plan;
 bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P);
 void pn_fused_plan_free(pn_fused_plan* pl);
 cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
+
+// periodic lateral faces (pn_wrap.cu): the wrap bonds' part of q and of the dot products; finishes alpha / beta
+cudaError_t pn_launch_wrap_fix(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st);
+cudaError_t pn_launch_wrap_copy(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 
 // Which iteration scheme a PN_OPT_KERNEL value selects on this lattice: 1 = reference two-kernel,
 // 2 = two-kernel with the TMA S4 kernel, 3 = single fused TMA kernel

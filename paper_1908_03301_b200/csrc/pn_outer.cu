@@ -31,6 +31,7 @@ __global__ void k_residual64(pn_geom g, pn_ptrs P, int fused) {
     __shared__ double tot[2];
     double a0 = 0.0, a1 = 0.0;
     float* __restrict__ rdst = (fused && (P.st->iters & 1)) ? P.r2 : P.r;
+    const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const float s = P.s[n];
         float rh = 0.f;
@@ -42,6 +43,18 @@ __global__ void k_residual64(pn_geom g, pn_ptrs P, int fused) {
             r += (double)P.gs[1][n - g.px] * (P.x64[n - g.px] - xc);
             r += (double)P.gs[2][n] * (P.x64[n + g.plane] - xc);
             r += (double)P.gs[2][n - g.plane] * (P.x64[n - g.plane] - xc);
+            if (wrap) {   // periodic lateral faces: the wrap bonds of a node on such a face
+                const int ci = (int)(n % g.px), cj = (int)((n / g.px) % g.ny), ck = (int)(n / g.plane);
+                for (int b = 0; b < 3; ++b) {
+                    if (!g.wrap[b]) continue;
+                    const int cb = b == 0 ? ci : (b == 1 ? cj : ck), db = b == 0 ? g.nx : (b == 1 ? g.ny : g.nz);
+                    if (cb != 0 && cb != db - 1) continue;
+                    const double gw = (double)P.gsw[b][pn_face_index(g, b, ci, cj, ck)];
+                    const long long span = pn_wrap_span(g, b);
+                    if (cb == 0) r += gw * (P.x64[n + span] - xc);
+                    if (cb == db - 1) r += gw * (P.x64[n - span] - xc);
+                }
+            }
             rh = (float)((double)s * r);
             a0 += r * r;
             a1 += (double)rh * (double)rh;

@@ -52,6 +52,28 @@ __device__ __forceinline__ coords coords_of(const pn_geom& g, long long n) {
 }
 __device__ __forceinline__ int along(const pn_geom& g, const coords& c) { return g.dir == 0 ? c.i : (g.dir == 1 ? c.j : c.k); }
 
+// Neighbour of padded node n along axis b (side 0: forward, 1: backward) and the storage of the bond between
+// them in the SOLVE COPY: the lattice-shaped array, or the face array when the step crosses a wrapping face
+// (periodic lateral faces).  A step off a face that does not wrap lands on a pad / halo entry whose
+// bond is 0, as everywhere in this layout.
+struct pn_nb { long long m; float* slot; };
+__device__ __forceinline__ pn_nb pn_nbr(const pn_geom& g, const pn_ptrs& P, long long n, const coords& c, int b, int side) {
+    const long long sb = b == 0 ? 1 : (b == 1 ? (long long)g.px : g.plane);
+    pn_nb r;
+    if (g.wrap[b]) {
+        const int cb = b == 0 ? c.i : (b == 1 ? c.j : c.k), db = b == 0 ? g.nx : (b == 1 ? g.ny : g.nz);
+        if ((side == 0 && cb == db - 1) || (side == 1 && cb == 0)) {
+            r.slot = P.gsw[b] + pn_face_index(g, b, c.i, c.j, c.k);
+            r.m = side == 0 ? n - pn_wrap_span(g, b) : n + pn_wrap_span(g, b);
+            return r;
+        }
+    }
+    r.m = side == 0 ? n + sb : n - sb;
+    r.slot = P.gs[b] + (side == 0 ? n : n - sb);
+    return r;
+}
+__device__ __forceinline__ bool any_wrap(const pn_geom& g) { return g.wrap[0] | g.wrap[1] | g.wrap[2]; }
+
 // ---- S1a: solve copy of g in the padded layout; union-find forest initialised -------------------
 // Off-lattice forward entries and pad columns -> 0.  Bonds lying INSIDE a Dirichlet plane (both ends
 // at the same fixed pressure, no current) -> 0.
@@ -76,6 +98,36 @@ __global__ void k_solve_copy(pn_geom g, pn_ptrs P) {
     }
 }
 
+// ---- periodic lateral faces: solve copy of the wrap bonds (face arrays) --------------------------------
+// gsw[b][f] = the caller's forward entry of the LAST node along b (the bond back to the first node); 0 on pad
+// columns and when both ends lie in a Dirichlet plane (no current, as for the in-plane bonds above).
+__global__ void k_wrap_copy(pn_geom g, pn_ptrs P) {
+    for (int b = 0; b < 3; ++b) {
+        if (!g.wrap[b]) { continue; }
+        const long long nf = pn_face_count(g, b);
+        for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+            coords c;   // the hi node of this face entry
+            if (b == 0) { c.i = g.nx - 1; c.j = (int)(f % g.ny); c.k = (int)(f / g.ny); }
+            else if (b == 1) { c.i = (int)(f % g.px); c.j = g.ny - 1; c.k = (int)(f / g.px); }
+            else { c.i = (int)(f % g.px); c.j = (int)(f / g.px); c.k = g.nz - 1; }
+            float v = 0.f;
+            const int ca = along(g, c);
+            if (c.i < g.nx && P.raw[b]) {
+                // with a wrapping axis this entry IS a bond: same validation as k_validate (S0), done here because
+                // which axes wrap is known only once the solve direction is
+                v = P.raw[b][c.i + (long long)g.nx * (c.j + (long long)g.ny * c.k)];
+                if (!(v >= 0.0f) || isinf(v)) atomicOr(&P.st->bad_value, 1);
+                if (v == 0.0f) atomicOr(&P.st->any_closed, 1);
+                if (ca == 0 || ca == g.n_a - 1) v = 0.f;
+            }
+            P.gsw[b][f] = v;
+        }
+    }
+}
+
+// unite the two ends of every open wrap bond (both are interior: Dirichlet-plane entries were zeroed)
+__global__ void k_wrap_union(pn_geom g, pn_ptrs P);
+
 // ---- union-find primitives (parent[] read at L2: another SM may have just re-hooked a root) -----
 __device__ __forceinline__ int uf_find(int* parent, int x) {
     int p = __ldcg(parent + x);
@@ -96,6 +148,47 @@ __device__ __forceinline__ void uf_union(int* parent, int a, int b) {
         const int old = atomicCAS(parent + a, a, b);  // hook the larger root under the smaller
         if (old == a) return;
         a = old;  // a stopped being a root meanwhile: carry on from its new parent
+    }
+}
+
+__global__ void k_wrap_union(pn_geom g, pn_ptrs P) {
+    for (int b = 0; b < 3; ++b) {
+        if (!g.wrap[b]) { continue; }
+        const long long nf = pn_face_count(g, b), span = pn_wrap_span(g, b);
+        for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+            if (!(P.gsw[b][f] > 0.f)) continue;
+            const long long lo = b == 0 ? (f % g.ny) * (long long)g.px + (f / g.ny) * g.plane
+                                        : (b == 1 ? (f % g.px) + (f / g.px) * g.plane : f);
+            uf_union(P.parent, (int)lo, (int)(lo + span));
+        }
+    }
+}
+
+// prune the wrap bonds: zero every one that has a pinned end
+__global__ void k_wrap_prune(pn_geom g, pn_ptrs P) {
+    for (int b = 0; b < 3; ++b) {
+        if (!g.wrap[b]) { continue; }
+        const long long nf = pn_face_count(g, b), span = pn_wrap_span(g, b);
+        for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+            if (P.gsw[b][f] == 0.f) continue;
+            const long long lo = b == 0 ? (f % g.ny) * (long long)g.px + (f / g.ny) * g.plane
+                                        : (b == 1 ? (f % g.px) + (f / g.px) * g.plane : f);
+            if (!(P.cls[lo] <= PN_CLASS_SOLVED && P.cls[lo + span] <= PN_CLASS_SOLVED)) P.gsw[b][f] = 0.f;
+        }
+    }
+}
+
+// scaled weights of the wrap bonds: ww = g s_lo s_hi (fp64 product, rounded once), as k_weights
+__global__ void k_wrap_weights(pn_geom g, pn_ptrs P) {
+    for (int b = 0; b < 3; ++b) {
+        if (!g.wrap[b]) { continue; }
+        const long long nf = pn_face_count(g, b), span = pn_wrap_span(g, b);
+        for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+            const long long lo = b == 0 ? (f % g.ny) * (long long)g.px + (f / g.ny) * g.plane
+                                        : (b == 1 ? (f % g.px) + (f / g.px) * g.plane : f);
+            const double v = (double)P.gsw[b][f];
+            P.ww[b][f] = v != 0.0 ? (float)(v * (double)P.s[lo] * (double)P.s[lo + span]) : 0.f;
+        }
     }
 }
 
@@ -203,40 +296,48 @@ __global__ void k_prune(pn_geom g, pn_ptrs P) {
 // dangling chain costs one walk, not one launch per node).  A node is claimed with atomicCAS(deg, 1, 0).
 __global__ void k_degree(pn_geom g, pn_ptrs P) {
     int* __restrict__ deg = P.flags;
+    const bool wrap = any_wrap(g);
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         int d = 0;
-        if (P.cls[n] == PN_CLASS_SOLVED)
-            d = (P.gs[0][n] != 0.f) + (P.gs[0][n - 1] != 0.f) + (P.gs[1][n] != 0.f) + (P.gs[1][n - g.px] != 0.f) +
-                (P.gs[2][n] != 0.f) + (P.gs[2][n - g.plane] != 0.f);
+        if (P.cls[n] == PN_CLASS_SOLVED) {
+            if (!wrap) {
+                d = (P.gs[0][n] != 0.f) + (P.gs[0][n - 1] != 0.f) + (P.gs[1][n] != 0.f) + (P.gs[1][n - g.px] != 0.f) +
+                    (P.gs[2][n] != 0.f) + (P.gs[2][n - g.plane] != 0.f);
+            } else {
+                const coords c = coords_of(g, n);
+                for (int b = 0; b < 3; ++b)
+                    for (int side = 0; side < 2; ++side) d += (*pn_nbr(g, P, n, c, b, side).slot != 0.f);
+            }
+        }
         deg[n] = d;
     }
 }
 
 __global__ void k_peel(pn_geom g, pn_ptrs P) {
     int* deg = P.flags;
-    const long long stride[3] = {1, g.px, g.plane};
     unsigned long long cnt = 0;
     for (long long n0 = blockIdx.x * (long long)blockDim.x + threadIdx.x; n0 < g.npad; n0 += (long long)gridDim.x * blockDim.x) {
         long long n = n0;
         while (__ldcg(deg + n) == 1 && atomicCAS(deg + n, 1, 0) == 1) {
             // the one bond left (bonds zeroed by other threads are read at L2: their stores were fenced
             // before the degree decrement that made this node a leaf)
+            const coords c = coords_of(g, n);
             int code = -1;
-#pragma unroll
-            for (int b = 0; b < 3; ++b) {
-                if (__ldcg(P.gs[b] + n) != 0.f) code = 2 * b;
-                if (__ldcg(P.gs[b] + n - stride[b]) != 0.f) code = 2 * b + 1;
-            }
+            pn_nb hit;
+            hit.m = -1; hit.slot = nullptr;
+            for (int b = 0; b < 3; ++b)
+                for (int side = 0; side < 2; ++side) {
+                    const pn_nb nb = pn_nbr(g, P, n, c, b, side);
+                    if (__ldcg(nb.slot) != 0.f) { code = 2 * b + side; hit = nb; }
+                }
             if (code < 0) break;
-            const long long sb = stride[code >> 1];
-            const long long m = (code & 1) ? n - sb : n + sb;
-            if (P.cls[m] != PN_CLASS_SOLVED) { deg[n] = 1; break; }   // hangs from a Dirichlet node: not a dead end
+            if (P.cls[hit.m] != PN_CLASS_SOLVED) { deg[n] = 1; break; }   // hangs from a Dirichlet node: not a dead end
             P.cls[n] = (signed char)(PN_CLASS_PEELED + code);
-            __stcg(P.gs[code >> 1] + ((code & 1) ? m : n), 0.f);
+            __stcg(hit.slot, 0.f);
             __threadfence();
             ++cnt;
-            if (atomicSub(deg + m, 1) != 2) break;                   // the neighbour did not become a leaf
-            n = m;
+            if (atomicSub(deg + hit.m, 1) != 2) break;                   // the neighbour did not become a leaf
+            n = hit.m;
         }
     }
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
@@ -246,28 +347,26 @@ __global__ void k_peel(pn_geom g, pn_ptrs P) {
 // Undo a peeling that removed too few nodes to pay (PN_OPT_PEEL = 2, see pn_api.cu): put every peeled node back
 // as an unknown and restore its bond from the caller's conductances.
 __global__ void k_unpeel(pn_geom g, pn_ptrs P) {
-    const long long stride[3] = {1, g.px, g.plane};
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const int c = P.cls[n];
         if (c < PN_CLASS_PEELED) continue;
-        const int code = c - PN_CLASS_PEELED, b = code >> 1;
-        const long long lo = (code & 1) ? n - stride[b] : n;      // the forward bond lives on its lower-index end
-        const coords cc = coords_of(g, lo);
-        P.gs[b][lo] = P.raw[b][cc.i + (long long)g.nx * (cc.j + (long long)g.ny * cc.k)];
+        const int code = c - PN_CLASS_PEELED, b = code >> 1, side = code & 1;
+        const pn_nb nb = pn_nbr(g, P, n, coords_of(g, n), b, side);
+        const coords cc = coords_of(g, side == 0 ? n : nb.m);      // the node whose FORWARD entry this bond is
+        *nb.slot = P.raw[b][cc.i + (long long)g.nx * (cc.j + (long long)g.ny * cc.k)];
         P.cls[n] = PN_CLASS_SOLVED;
     }
 }
 
 // After the solve: every peeled node takes the pressure of the unpeeled node its dangling tree hangs from.
 __global__ void k_backfill(pn_geom g, pn_ptrs P) {
-    const long long stride[3] = {1, g.px, g.plane};
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         int c = P.cls[n];
         if (c < PN_CLASS_PEELED) continue;
         long long m = n;
         for (long long guard = 0; c >= PN_CLASS_PEELED && guard < g.npad; ++guard) {
             const int code = c - PN_CLASS_PEELED;
-            m += (code & 1) ? -stride[code >> 1] : stride[code >> 1];
+            m = pn_nbr(g, P, m, coords_of(g, m), code >> 1, code & 1).m;
             c = P.cls[m];
         }
         P.x64[n] = P.x64[m];
@@ -284,10 +383,15 @@ __global__ void k_scale(pn_geom g, pn_ptrs P) {
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         float s = 0.f;
         if (P.cls[n] == PN_CLASS_SOLVED) {
-            const double d = (double)P.gs[0][n] + (double)P.gs[0][n - 1] + (double)P.gs[1][n] + (double)P.gs[1][n - g.px] +
-                             (double)P.gs[2][n] + (double)P.gs[2][n - g.plane];
-            s = d > 0.0 ? (float)(1.0 / sqrt(d)) : 0.f;
             const coords c = coords_of(g, n);
+            double d = (double)P.gs[0][n] + (double)P.gs[0][n - 1] + (double)P.gs[1][n] + (double)P.gs[1][n - g.px] +
+                       (double)P.gs[2][n] + (double)P.gs[2][n - g.plane];
+            for (int b = 0; b < 3; ++b) {   // wrap bonds of a node on a periodic face (the lattice arrays hold 0 there)
+                if (!g.wrap[b]) continue;
+                const int cb = b == 0 ? c.i : (b == 1 ? c.j : c.k), db = b == 0 ? g.nx : (b == 1 ? g.ny : g.nz);
+                if (cb == 0 || cb == db - 1) d += (double)P.gsw[b][pn_face_index(g, b, c.i, c.j, c.k)];
+            }
+            s = d > 0.0 ? (float)(1.0 / sqrt(d)) : 0.f;
             if (along(g, c) == 1) { const double b = (double)P.gs[g.dir][n - g.stride_a]; bb += b * b; }
         }
         P.s[n] = s;
@@ -325,13 +429,19 @@ cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t 
 cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, bool do_peel, int x0_linear,
                             cudaStream_t st, int* launches) {
     const int nb = grid_for(g.npad);
+    const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];
+    long long nface = 1;
+    for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
+    const int nbf = grid_for(nface);
     k_solve_copy<<<nb, TPB, 0, st>>>(g, P);
     ++*launches;
     if (do_label) {
         k_union<<<nb, TPB, 0, st>>>(g, P);
+        if (wrap) { k_wrap_union<<<nbf, TPB, 0, st>>>(g, P); ++*launches; }
         k_touch<<<nb, TPB, 0, st>>>(g, P);
         k_classify<true><<<nb, TPB, 0, st>>>(g, P, x0_linear);
         k_prune<<<nb, TPB, 0, st>>>(g, P);
+        if (wrap) { k_wrap_prune<<<nbf, TPB, 0, st>>>(g, P); ++*launches; }
         *launches += 4;
         if (do_peel) {
             k_degree<<<nb, TPB, 0, st>>>(g, P);
@@ -351,6 +461,12 @@ cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st,
     k_scale<<<nb, TPB, 0, st>>>(g, P);
     k_weights<<<nb, TPB, 0, st>>>(g, P);
     *launches += 2;
+    if (g.wrap[0] || g.wrap[1] || g.wrap[2]) {
+        long long nface = 1;
+        for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
+        k_wrap_weights<<<grid_for(nface), TPB, 0, st>>>(g, P);
+        ++*launches;
+    }
     return cudaGetLastError();
 }
 
@@ -362,6 +478,16 @@ cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t 
 
 cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
     k_unpeel<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+// Periodic lateral faces: solve copy of the wrap bonds + their validation (sets state.bad_value / any_closed).
+// Runs before pn_launch_label so that the host can read the two flags first.
+cudaError_t pn_launch_wrap_copy(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    long long nface = 1;
+    for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
+    k_wrap_copy<<<grid_for(nface), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }

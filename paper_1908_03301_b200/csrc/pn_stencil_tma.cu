@@ -62,13 +62,6 @@ struct alignas(64) pn_tmaps {
     CUtensorMap r_main, r_slv, p_main[2], p_slv[2], xh, wx_main, wx_slv, wy, wz;
 };
 
-// epilogue shared with the reference kernel (pn_inner.cu keeps its own copy: same arithmetic)
-__device__ __forceinline__ void finish_A(pn_state* st, double pq) {
-    st->pq = pq;
-    if (st->rr == 0.0) st->flag = PN_FLAG_CONVERGED;
-    else if (!(pq > 0.0) || isinf(pq)) st->flag = PN_FLAG_BREAKDOWN;
-    else st->alpha = st->rr / pq;
-}
 
 template <class C>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
@@ -253,7 +246,10 @@ k_stencil_tma(const __grid_constant__ pn_tmaps maps, pn_geom g, pn_ptrs P, int n
     acc = pn_block_sum(acc, red);
     const double v1[1] = {acc};
     if (pn_grid_sum<1>(v1, P.slots, &st->ticket, red, red + 32)) {
-        if (threadIdx.x == 0) finish_A(st, red[32]);
+        if (threadIdx.x == 0) {
+            if (g.wrap[0] | g.wrap[1] | g.wrap[2]) st->part[0] = red[32];   // periodic faces: k_wrap_fix finishes
+            else pn_finish_A(st, red[32]);
+        }
     }
 }
 

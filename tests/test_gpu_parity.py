@@ -44,8 +44,11 @@ def gpu_solve(pn, net, direction, tol, opts=None):
     return info, P, cls, fl, n_launch
 
 
-def compare(pn, oracle, net, direction, tol=1e-12, opts=None):
-    ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13)
+def compare(pn, oracle, net, direction, tol=1e-12, opts=None, periodic=False):
+    ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13, periodic=periodic)
+    if periodic:
+        opts = dict(opts or {})
+        opts[pn.PN_OPT_LATERAL] = 1
     info, P, cls, fl, n_launch = gpu_solve(pn, net, direction, tol, opts)
     assert n_launch > 0
     # integer work: classes bit-exact, counts equal
@@ -431,3 +434,85 @@ def test_peeling_automatic_policy(pn, oracle):
     never, P_never, fl_never, _ = compare(pn, oracle, far, 0, opts={pn.PN_OPT_PEEL: 0})
     assert auto.inner_iters == never.inner_iters
     assert np.array_equal(P_auto, P_never) and fl_auto == fl_never
+
+
+# ---- periodic lateral faces: PN_OPT_LATERAL = 1 against the oracle's periodic=True ----
+@pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 2, 7), (12, 6, 2)])
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("p", [1.0, 0.6])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
+def test_periodic_ragged_3d(pn, oracle, shape, direction, p, kernel):
+    """All three kernel schemes; lateral axes of length 2 (a doubled bond) included."""
+    from paper_1908_03301_b200 import inputs
+    if shape[direction] < 3:
+        pytest.skip("solve axis needs 3 node planes")
+    net = inputs.iid_diluted(*shape, seed=17 + direction, p=p)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
+
+
+@pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (257, 31)])
+@pytest.mark.parametrize("direction", [0, 1])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
+def test_periodic_ragged_2d(pn, oracle, shape, direction, kernel):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(shape[0], shape[1], 1, seed=13 + direction, p=0.75)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
+
+
+@pytest.mark.parametrize("kernel", [2, 3])
+@pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
+def test_periodic_multi_tile(pn, oracle, shape, direction, kernel):
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(*shape, seed=6, p=0.75)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
+
+
+def test_periodic_config_siblings(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    compare(pn, oracle, inputs.cfg2_fbm_2d(256, 256), 0, periodic=True)
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13, periodic=True)    # automatic: fused TMA kernel
+    info, P, fl, ref = compare(pn, oracle, inputs.cfg3_percolation_3d(64, 64, 64), 0, periodic=True)
+    from oracle import pn_oracle as po
+    net = inputs.cfg3_percolation_3d(64, 64, 64)
+    wrap = po.wrap_axes(64, 64, 64, 0, True)
+    g64 = po.widen(64, 64, 64, net.gx, net.gy, net.gz, wrap)
+    assert info.n_peeled == int(po.dangling_ends(64, 64, 64, g64, ref.classes, wrap).sum()) > 0
+
+
+def test_periodic_closed_forms(pn):
+    """Hand-worked golden example (tests/golden/worked_3x2_periodic.txt) and the uniform network."""
+    gx = np.array([[[1, 2, 99], [3, 4, 99]]], dtype=np.float32)
+    gy = np.array([[[77, 5, 77], [88, 7, 88]]], dtype=np.float32)
+    h = pn.Network(3, 2, 1)
+    h.set_option(pn.PN_OPT_LATERAL, 1)
+    h.set_conductances(gx, gy, None)
+    h.solve(0, 1e-13)
+    P = h.pressures().cpu().numpy()
+    fl = h.flux()
+    h.close()
+    assert P[0, 0, 1] == pytest.approx(55 / 141, abs=1e-13)
+    assert P[0, 1, 1] == pytest.approx(57 / 141, abs=1e-13)
+    assert fl[0] == pytest.approx(338 / 141, rel=1e-12) and fl[1] == pytest.approx(338 / 141, rel=1e-12)
+    from paper_1908_03301_b200 import inputs
+    net = inputs.uniform(9, 6, 5, 0.37)
+    for d in range(3):
+        info, P, cls, fl, _ = gpu_solve(pn, net, d, 1e-12, opts={pn.PN_OPT_LATERAL: 1})
+        n_a = (9, 6, 5)[d]
+        assert fl[2] == pytest.approx(np.float64(np.float32(0.37)) * (270 // n_a) / (n_a - 1), rel=1e-12)
+
+
+def test_periodic_validates_wrap_entries(pn):
+    """With wrapping axes the forward entry of a last node is a bond: a NaN there is PN_ERR_VALUE at pn_solve, and
+    is still ignored with no-flux faces."""
+    g = np.ones((4, 6, 8), dtype=np.float32)
+    bad = g.copy()
+    bad[2, 5, 3] = np.nan                      # gy of the last row: off-lattice unless y wraps
+    h = pn.Network(8, 6, 4)
+    h.set_conductances(g, bad, g)
+    h.solve(0, 1e-10)
+    h.set_option(pn.PN_OPT_LATERAL, 1)
+    with pytest.raises(pn.PnError) as e:
+        h.solve(0, 1e-10)
+    assert e.value.code == pn.PN_ERR_VALUE
+    h.solve(1, 1e-10)                          # y is the solve axis: it does not wrap, the entry is ignored again
+    h.close()
