@@ -101,6 +101,8 @@ enum {
                                the forward entry of the LAST node along such an axis is the bond back to the
                                first node (validated at pn_solve: PN_ERR_VALUE).  An axis of one node does
                                not wrap                                                             */
+    PN_OPT_GRAPH = 9,       /* 1 (default): a chunk of inner iterations is replayed from a CUDA graph (captured
+                               once per geometry / direction / scheme); 0: every kernel launched directly  */
     PN_OPT_PEEL = 7         /* dead-end peeling: solved nodes left with one open bond carry no current
                                (S8(c) reading 7, S8(f) item 1); they are removed from the system,
                                recursively, and take the pressure of the node they hang from after the

@@ -35,6 +35,12 @@ struct pn_ctx {
     // options
     int max_iters, chunk, x0_linear, skip_label, variant, profile, peel, lateral;
     int base_closed;            // some in-lattice (non-wrap) bond is closed: from S0's validation
+    // CUDA graph of one chunk of inner iterations (captured on a private stream, launched on the caller's)
+    int use_graph;
+    cudaStream_t cap_stream;
+    cudaGraphExec_t graph_exec;
+    pn_geom graph_g;
+    int graph_scheme, graph_chunk;
     cudaEvent_t* pev;           // event pool for PN_OPT_PROFILE (2*chunk+1), created on demand
     int pev_n;
     double delta;
@@ -152,7 +158,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1;
     ctx->delta = 0.1;
     ctx->last_dir_user = -1;
     cudaDeviceProp prop;
@@ -204,6 +210,8 @@ int pn_destroy(pn_ctx* ctx) {
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     for (int i = 0; i < ctx->pev_n; ++i) cudaEventDestroy(ctx->pev[i]);
     delete[] ctx->pev;
+    if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
     return PN_OK;
 }
@@ -219,6 +227,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
+        case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
@@ -277,6 +286,41 @@ static int read_state(pn_ctx* ctx) {
     CK(cudaMemcpyAsync(ctx->h_state, ctx->P.st, sizeof(pn_state), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return PN_OK;
+}
+
+// One chunk of inner iterations as a CUDA graph: the launches carry no per-iteration host arguments (buffer
+// parity, alpha, beta and the run flag are read on the device), so the same executable graph serves every chunk
+// of a solve and every later solve with the same geometry, direction, scheme and chunk length.  Captured on a
+// private stream (the caller's may be the legacy default stream, which cannot be captured); nothing executes
+// there.  Returns false (graph_exec == nullptr) when capture is unavailable: the caller launches directly.
+static bool ensure_graph(pn_ctx* ctx, int scheme) {
+    if (ctx->graph_exec && ctx->graph_scheme == scheme && ctx->graph_chunk == ctx->chunk &&
+        memcmp(&ctx->graph_g, &ctx->g, sizeof(pn_geom)) == 0)
+        return true;
+    if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
+    if (!ctx->cap_stream && cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        ctx->cap_stream = nullptr;
+        cudaGetLastError();
+        return false;
+    }
+    int dummy = 0;
+    // warm the launch path once outside capture is not needed: function attributes are set by the launchers themselves
+    if (cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return false; }
+    cudaError_t e = pn_launch_inner(ctx->g, ctx->P, ctx->chunk, scheme, ctx->cap_stream, &dummy, nullptr);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e2 = cudaStreamEndCapture(ctx->cap_stream, &graph);
+    if (e != cudaSuccess || e2 != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return false;
+    }
+    e = cudaGraphInstantiate(&ctx->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { ctx->graph_exec = nullptr; cudaGetLastError(); return false; }
+    ctx->graph_g = ctx->g;
+    ctx->graph_scheme = scheme;
+    ctx->graph_chunk = ctx->chunk;
+    return true;
 }
 
 int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
@@ -385,11 +429,28 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         double best_rn = rn;
         int stagnant = 0;
         int iters_seen = 0;
+        // Graph path: whole chunks replayed from one executable graph.  With PN_OPT_PROFILE it is used for the single-kernel
+        // scheme only (one kernel per iteration: the chunk's device time / iterations run is that kernel's average launch
+        // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
+        const bool graph = ctx->use_graph && ctx->chunk > 1 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme);
+        const int per_iter = (fused ? 1 : 2) + (any_wrap ? 1 : 0);
         while (true) {
-            CK(pn_launch_inner(g, P, ctx->chunk, scheme, s, &nl, ctx->profile ? ctx->pev : nullptr));
+            if (graph) {
+                if (ctx->profile) CK(cudaEventRecord(ctx->pev[0], s));
+                CK(cudaGraphLaunch(ctx->graph_exec, s));
+                if (ctx->profile) CK(cudaEventRecord(ctx->pev[1], s));
+                nl += per_iter * ctx->chunk;
+            } else {
+                CK(pn_launch_inner(g, P, ctx->chunk, scheme, s, &nl, ctx->profile ? ctx->pev : nullptr));
+            }
             rc = read_state(ctx);
             if (rc) return rc;
-            if (ctx->profile) {   // per-kernel device time of the launches that did work (not the no-op tail)
+            if (ctx->profile && graph) {
+                const int ran = h->iters - iters_seen;
+                float ta = 0.f;
+                cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
+                if (ran > 0) { t_stencil += ta; n_timed += ran; }
+            } else if (ctx->profile) {   // per-kernel device time of the launches that did work (not the no-op tail)
                 const int ran = h->iters - iters_seen;
                 for (int it = 0; it < ran && it < ctx->chunk; ++it) {
                     float ta = 0.f, tb = 0.f;

@@ -70,13 +70,15 @@ def _f32(a) -> np.ndarray:
 # Fractional-Brownian-motion field by spectral synthesis (eq.(1), generalised to d
 # dimensions as S(k) ~ |k|^-(2H+d), SURVEY.md 8(c) readings 12-13).
 # --------------------------------------------------------------------------------------------------
-def fbm_fields(shape: tuple, H: float, rng: np.random.Generator, bond_axes=()) -> tuple:
+def fbm_fields(shape: tuple, H: float, rng: np.random.Generator, bond_axes=(), beta=None) -> tuple:
     """Node-centred FBM field `B0` and, for each axis in `bond_axes`, the same realisation sampled at
     the midpoints of the bonds along that axis (half-cell Fourier shift).
 
     white noise w -> W = fftn(w) -> W * |k|^-(H + d/2) with k_i = m_i / n_i (cycles per sample), the
     k = 0 mode and every Nyquist plane (even n) zeroed -> inverse FFT.  All fields are normalised with
     the NODE field's mean and standard deviation.  Periodic on the box, no padding.
+    `beta` (one positive number per array axis): the anisotropic spectrum of PAPER.md:33-35 eq.(2),
+    S ~ (sum_a beta_a k_a^2)^-(H + d/2); None = isotropic, eq.(1).
     Returns (B0, {axis: B_axis}); axes index the array dimensions of `shape` (C order).
     """
     shape = tuple(int(s) for s in shape)
@@ -90,7 +92,7 @@ def fbm_fields(shape: tuple, H: float, rng: np.random.Generator, bond_axes=()) -
         f = sfft.fftfreq(n)                      # m / n, signed
         sl = [None] * len(shape)
         sl[ax] = slice(None)
-        k2 = k2 + (f * f)[tuple(sl)]
+        k2 = k2 + (1.0 if beta is None else float(beta[ax])) * (f * f)[tuple(sl)]
         if n % 2 == 0 and n > 1:
             nyq = np.zeros(n, dtype=bool)
             nyq[n // 2] = True
@@ -139,6 +141,21 @@ def cfg2_fbm_2d(nx: int = 2048, ny: int = 2048, seed: int = 1, H: float = 0.7,
     gy = np.exp(sigma * B[0]).reshape(_shape(nx, ny, 1))
     return Network(nx, ny, 1, _f32(gx), _f32(gy), None, (0,), False,
                    f"cfg2_fbm2d_{nx}x{ny}_H{H}_s{seed}")
+
+
+def aniso_fbm_2d(nx: int, ny: int, seed: int, H: float, beta_x: float, beta_y: float = 1.0,
+                 sigma: float = 1.0) -> Network:
+    """2D FBM log-conductance with the ANISOTROPIC spectrum of PAPER.md:33-37 eq.(2),
+    S = b / (beta_x w_x^2 + beta_y w_y^2)^(H+1); g = exp(sigma * B) at bond midpoints as in CFG2.
+    beta_x / beta_y > 1 damps the variation along x: layers parallel to x.  Solved along x and y
+    for the permeability anisotropy K_x / K_y of Fig.10.  beta_x = beta_y reproduces cfg2_fbm_2d."""
+    r = _rng(seed)
+    _, B = fbm_fields((ny, nx), H, r, bond_axes=(1, 0), beta=(beta_y, beta_x))
+    gx = np.exp(sigma * B[1]).reshape(_shape(nx, ny, 1))
+    gy = np.exp(sigma * B[0]).reshape(_shape(nx, ny, 1))
+    return Network(nx, ny, 1, _f32(gx), _f32(gy), None, (0, 1), False,
+                   f"anisofbm2d_{nx}x{ny}_H{H}_bx{beta_x}_by{beta_y}_s{seed}",
+                   {"H": H, "beta_x": beta_x, "beta_y": beta_y, "sigma": sigma})
 
 
 def cfg3_percolation_3d(nx: int = 256, ny: int = 256, nz: int = 256, seed: int = 2,

@@ -24,7 +24,7 @@ LIB_PATH = os.path.join(HERE, "libpn.so")
 PN_OK, PN_NO_SPANNING_CLUSTER, PN_MAX_ITERS = 0, 1, 2
 PN_ERR_ARG, PN_ERR_STATE, PN_ERR_VALUE, PN_ERR_WORKSPACE, PN_ERR_CUDA, PN_ERR_BREAKDOWN = -1, -2, -3, -4, -5, -6
 (PN_OPT_MAX_ITERS, PN_OPT_DELTA, PN_OPT_X0, PN_OPT_CHUNK, PN_OPT_SKIP_LABEL, PN_OPT_KERNEL, PN_OPT_PROFILE,
- PN_OPT_PEEL, PN_OPT_LATERAL) = range(9)
+ PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH) = range(10)
 CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CLASS_FLOATING = range(6)
 
 # every symbol include/pn.h declares (tests check that the library exports each of them)

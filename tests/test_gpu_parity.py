@@ -516,3 +516,38 @@ def test_periodic_validates_wrap_entries(pn):
     assert e.value.code == pn.PN_ERR_VALUE
     h.solve(1, 1e-10)                          # y is the solve axis: it does not wrap, the entry is ignored again
     h.close()
+
+
+def test_anisotropic_fbm_both_directions(pn, oracle):
+    """Eq.(2) input (S8(f) item 3), periodic faces, x and y solves on one handle: parity in both directions, and
+    layers parallel to x (beta_x / beta_y = 16) conduct better along x than across."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.aniso_fbm_2d(160, 128, 3, 0.75, 4.0, 0.25)
+    k = []
+    for d in net.directions:
+        info, P, fl, ref = compare(pn, oracle, net, d, periodic=True)
+        k.append(fl[3])
+        assert fl[3] == pytest.approx(ref.k_eff, rel=1e-9)
+    assert k[0] > k[1]
+
+
+@pytest.mark.parametrize("kernel", [1, 3])
+def test_graph_replay_is_bit_identical(pn, kernel):
+    """PN_OPT_GRAPH: replaying chunks from a CUDA graph launches the same kernels on the same data -- pressures,
+    fluxes and iteration counts are identical to direct launches; the graph is reused across solves of one handle."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg3_percolation_3d(48, 48, 48)
+    a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 1})
+    b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 0})
+    assert a[0].inner_iters == b[0].inner_iters and a[0].outer_cycles == b[0].outer_cycles
+    assert np.array_equal(a[1], b[1]) and a[3] == b[3]
+    assert a[4] == b[4]                                   # same launch count
+    h = pn.Network(net.nx, net.ny, net.nz)
+    h.set_option(pn.PN_OPT_KERNEL, kernel)
+    h.set_conductances(net.gx, net.gy, net.gz)
+    for d in (0, 1, 0, 2):                                # direction changes force a re-capture
+        h.solve(d, 1e-10)
+        P = h.pressures().cpu().numpy()
+        ref = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 0})
+        assert np.array_equal(P, ref[1])
+    h.close()

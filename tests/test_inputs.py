@@ -72,3 +72,16 @@ def test_transpose_axes_moves_bonds_with_their_axis():
     # new x bond at new (i',j',k') = old y bond at old (i=k', j=i', k=j')
     assert t.gx[1, 0, 2] == n.gy[0, 2, 1]
     assert (t.nx, t.ny, t.nz) == (3, 2, 4)
+
+
+def test_anisotropic_fbm_recipe():
+    """PAPER.md:33-37 eq.(2): beta_x = beta_y is CFG2's isotropic recipe bit for bit; beta_x / beta_y > 1 gives
+    layers parallel to x (the field varies less along x than along y); seeded, so reproducible."""
+    a = inputs.cfg2_fbm_2d(64, 48, seed=5)
+    b = inputs.aniso_fbm_2d(64, 48, 5, 0.7, 1.0, 1.0)
+    assert np.array_equal(a.gx, b.gx) and np.array_equal(a.gy, b.gy)
+    c = inputs.aniso_fbm_2d(128, 128, 5, 0.75, 16.0, 1.0)
+    B = np.log(c.gx[0].astype(np.float64))
+    assert np.var(np.diff(B, axis=1)) < 0.3 * np.var(np.diff(B, axis=0))
+    d = inputs.aniso_fbm_2d(128, 128, 5, 0.75, 16.0, 1.0)
+    assert c.sha256() == d.sha256() and c.directions == (0, 1)
