@@ -89,7 +89,7 @@ enum {
     PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32)            */
     PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
-    PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (3 on lattices of >= 2^21 nodes, else 1),
+    PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept for cross-checks and small lattices), 2 = TMA-fed 2.5D S4 kernel
                                + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused)      */

@@ -105,7 +105,7 @@ def test_cfg5_sibling(pn, oracle, direction):
 
 
 def test_cfg4_sibling_128(pn, oracle):
-    """2^21 nodes: the size from which the automatic choice is the TMA kernel."""
+    """2^21 nodes, tol 1e-13: several tiles in x and y and several z chunks with default options."""
     from paper_1908_03301_b200 import inputs
     compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13)
 
