@@ -71,7 +71,8 @@ typedef struct {
                               of the single fused S4+S5+S6 kernel; t_update_ms is then 0) ...       */
     double t_update_ms;    /* ... and of the S5 kernel launches (CUDA events on the handle's stream) */
     int n_timed_iters;     /* ... over this many inner iterations                                   */
-    int reserved2;
+    int n_xskip;           /* single-kernel scheme: inner iterations that skipped the x_hat update (PN_OPT_XDEFER):
+                              they move 8 bytes per node less than the others                        */
     long long n_peeled;    /* solved nodes taken out of the system as dangling ends (PN_OPT_PEEL) and
                               back-filled after the solve; they are counted in n_solved too           */
 } pn_info;
@@ -103,6 +104,9 @@ enum {
                                not wrap                                                             */
     PN_OPT_GRAPH = 9,       /* 1 (default): a chunk of inner iterations is replayed from a CUDA graph (captured
                                once per geometry / direction / scheme); 0: every kernel launched directly  */
+    PN_OPT_XDEFER = 10,     /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
+                               iteration, two search directions at once (the earlier one recovered from p and r):
+                               40 instead of 44 bytes per node-iteration on average; 0: every iteration    */
     PN_OPT_PEEL = 7         /* dead-end peeling: solved nodes left with one open bond carry no current
                                (S8(c) reading 7, S8(f) item 1); they are removed from the system,
                                recursively, and take the pressure of the node they hang from after the

@@ -36,7 +36,7 @@ struct pn_ctx {
     int max_iters, chunk, x0_linear, skip_label, variant, profile, peel, lateral;
     int base_closed;            // some in-lattice (non-wrap) bond is closed: from S0's validation
     // CUDA graph of one chunk of inner iterations (captured on a private stream, launched on the caller's)
-    int use_graph;
+    int use_graph, xdefer;
     cudaStream_t cap_stream;
     cudaGraphExec_t graph_exec;
     pn_geom graph_g;
@@ -158,7 +158,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1;
     ctx->delta = 0.1;
     ctx->last_dir_user = -1;
     cudaDeviceProp prop;
@@ -228,6 +228,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
+        case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
@@ -419,13 +420,14 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         rn = 0.0;
     } else if (rn > tol * nb) {
         const double delta2 = ctx->delta * ctx->delta;
+        const double xskip_min = (fused && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
         auto target_for = [&](double rn_true, double rr_true) {
             // proxy of the fp64 exit test in the scaled norm: ||r|| / ||r_hat|| measured at this replacement
             const double c = rn_true / sqrt(rr_true);
             const double t = 0.7 * tol * nb / c;
             return t * t;
         };
-        CK(pn_launch_set_state(P, rr_hat, 0.0, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 1, s, &nl));
+        CK(pn_launch_set_state(P, rr_hat, 0.0, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 1, xskip_min, s, &nl));
         double best_rn = rn;
         int stagnant = 0;
         int iters_seen = 0;
@@ -483,7 +485,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
             if (!(rr_hat > 0.0)) { status = PN_MAX_ITERS; break; }
             // continue the same Krylov sequence: beta = (true r.r) / (r.r before the last step)
             const double beta = rr_before > 0.0 ? rr_hat / rr_before : 0.0;
-            CK(pn_launch_set_state(P, rr_hat, beta, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 0, s, &nl));
+            CK(pn_launch_set_state(P, rr_hat, beta, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 0, xskip_min, s, &nl));
         }
     }
     if (n_peeled > 0) CK(pn_launch_backfill(g, P, s, &nl));   // dangling ends take the pressure of the node they hang from
@@ -499,6 +501,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         info->outer_cycles = outer;
         info->inner_iters = total_iters;
         info->kernel_scheme = scheme;
+        info->n_xskip = h->n_xskip;
         info->rel_residual = nb > 0.0 ? rn / nb : 0.0;
         info->b_norm = nb;
         info->n_solved = n_solved;

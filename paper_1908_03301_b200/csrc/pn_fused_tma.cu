@@ -83,6 +83,11 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     const float al = (float)st->alpha;          // alpha_{t-1} (0 right after a residual replacement)
     const float nal = -al;
     const int par = st->iters & 1;              // buffers holding r_{t-1}, q_{t-1}, p_{t-1}
+    // x_hat is touched every OTHER iteration: xmode 0 = skip (alpha_{t-1} p_{t-1} stays owed), 2 = apply this
+    // iteration's update and the owed one, whose direction is recovered as p_{t-2} = (p_{t-1} - r_{t-1}) / beta_{t-1}
+    // from values this kernel loads anyway; 1 = plain update (skipping disabled, or beta too small to divide by).
+    const int xmode = st->xpend ? 2 : ((st->xskip_min > 0.0 && st->beta >= st->xskip_min) ? 0 : 1);
+    const float c2 = xmode == 2 ? (float)(st->alpha2 / st->beta_prev) : 0.f;
     float* __restrict__ r_out = par ? P.r : P.r2;
     float* __restrict__ q_out = par ? P.q : P.q2;
     float* __restrict__ p_out = par ? P.p : P.p2;
@@ -173,14 +178,14 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
             float4 wzm = make_float4(0.f, 0.f, 0.f, 0.f);
             float4 r_cur = make_float4(0.f, 0.f, 0.f, 0.f);     // r_t on the own float4 of plane kk
             float4 xh_nxt = make_float4(0.f, 0.f, 0.f, 0.f);    // x_hat of plane kk+1, fetched one step ahead
-            if (inb) xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)k0 * g.plane + nrow);
+            if (inb && xmode) xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)k0 * g.plane + nrow);
             bar_consumers(C::NCONS);   // the ring is rebuilt per item: nobody may still read the previous item's planes
             for (int kk = k0 - 2; kk < k1; ++kk, ++it) {
                 const int s = it % C::S;
                 const unsigned ph = (it / C::S) & 1u;
                 // x_hat of plane kk+2 goes in flight now and is used one step later
                 const float4 xh_use = xh_nxt;
-                if (inb && kk + 2 >= k0 + 1 && kk + 2 < k1)
+                if (inb && xmode && kk + 2 >= k0 + 1 && kk + 2 < k1)
                     xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)(kk + 2) * g.plane + nrow);
                 mbar_wait(full + s, ph);
                 const float* sg = stages + s * C::STAGE_FLOATS;
@@ -189,14 +194,21 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 float4 r_nxt;
                 {
                     const float4 po = lds4(sg + C::P_ + own_main);
-                    r_nxt = fma4(nal, lds4(sg + C::Q_ + own_main), lds4(sg + C::R_ + own_main));
+                    const float4 ro = lds4(sg + C::R_ + own_main);      // r_{t-1}
+                    r_nxt = fma4(nal, lds4(sg + C::Q_ + own_main), ro);
                     const float4 pn = fma4(beta, po, r_nxt);
                     *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
                     if (kk + 1 >= k0 && kk + 1 < k1 && inb) {
                         const long long n = (long long)(kk + 1) * g.plane + nrow;
                         *reinterpret_cast<float4*>(r_out + n) = r_nxt;
                         *reinterpret_cast<float4*>(p_out + n) = pn;
-                        *reinterpret_cast<float4*>(P.xh + n) = fma4(al, po, xh_use);
+                        if (xmode) {
+                            float4 xn = fma4(al, po, xh_use);
+                            if (xmode == 2)
+                                xn = make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
+                                                 fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
+                            *reinterpret_cast<float4*>(P.xh + n) = xn;
+                        }
                         a_rr += (double)dot4(r_nxt, r_nxt);
                     }
                 }

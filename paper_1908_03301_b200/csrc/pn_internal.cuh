@@ -58,6 +58,12 @@ struct pn_state {
     double rr_max;              // largest rr since the last fp64 residual replacement
     double rr_target;           // proxy exit threshold on rr (set by the host from tol)
     double delta2;              // reliable-update threshold squared
+    // single-kernel scheme: the x_hat update is applied every OTHER iteration (two search directions at once)
+    double alpha2;              // alpha of the skipped update (pending on the direction before the current one)
+    double beta_prev;           // beta that built the current direction from the skipped one
+    double xskip_min;           // skip only while beta >= this (0: never skip)
+    int xpend;                  // 1: the previous kernel skipped its x_hat update
+    int n_xskip;                // iterations of this solve that skipped it (36 instead of 44 B per node)
     double part[4];             // periodic faces: the main kernel's sums, finished by k_wrap_fix (rr, pq, rq, qq | pq)
     double acc[4];              // results of the fp64 reductions (residual norms, b norm, flux)
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
@@ -103,6 +109,16 @@ __device__ __forceinline__ void pn_finish_F(pn_state* st, double rr, double pq, 
         else if (it >= st->max_iters) flag = PN_FLAG_BUDGET;
         else if (!(rr_next > 0.0) || isinf(rr_next)) flag = PN_FLAG_UPDATE;   // prediction lost: replace the residual
         else beta = rr_next / rr;
+    }
+    // the kernel that just ran skipped its x_hat update iff nothing was pending and its beta allowed the recovery
+    // p_{t-1} = (p_t - r_t) / beta_t later (same test as in k_cg_fused_tma)
+    if (!st->xpend && st->xskip_min > 0.0 && st->beta >= st->xskip_min) {
+        st->xpend = 1;
+        st->n_xskip += 1;
+        st->alpha2 = st->alpha;       // alpha_{t-1}, still owed on p_{t-1}
+        st->beta_prev = st->beta;     // beta_t
+    } else {
+        st->xpend = 0;
     }
     st->alpha = alpha;      // alpha_t: next kernel's residual and solution updates
     st->alpha_x = alpha;    // ... and what k_flush applies to the pending direction p_t
@@ -191,7 +207,8 @@ cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t 
 cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches);
 cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,
-                                double delta2, int max_iters, int reset_iters, cudaStream_t st, int* launches);
+                                double delta2, int max_iters, int reset_iters, double xskip_min, cudaStream_t st,
+                                int* launches);
 cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int variant, cudaStream_t st,
                             int* launches, cudaEvent_t* ev);
 cudaError_t pn_launch_flux(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);

@@ -70,18 +70,31 @@ __global__ void k_residual64(pn_geom g, pn_ptrs P, int fused) {
 }
 
 // ---- S7: x64 += s * (x_hat + alpha_x p)  (the pending deferred update included); x_hat = 0 ------
+// Single-kernel scheme with a skipped x_hat update pending (state.xpend): the direction before the last one is
+// recovered as p_{T-1} = (p_T - r_T) / beta_T from the last kernel's p and r, exactly as the next kernel would have.
 __global__ void k_flush(pn_geom g, pn_ptrs P) {
     const double ax = P.st->alpha_x;
     const float* __restrict__ p = (P.st->iters & 1) ? P.p2 : P.p;   // the direction of the last iteration
+    const float* __restrict__ r = (P.st->iters & 1) ? P.r2 : P.r;   // single-kernel scheme: the residual it was built from
+    const bool pend = P.st->xpend != 0;
+    const double c2 = pend ? P.st->alpha2 / P.st->beta_prev : 0.0;
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const float s = P.s[n];
-        if (s != 0.f) P.x64[n] += (double)s * ((double)P.xh[n] + ax * (double)p[n]);
+        if (s != 0.f) {
+            double dx = (double)P.xh[n] + ax * (double)p[n];
+            if (pend) dx += c2 * ((double)p[n] - (double)r[n]);
+            P.x64[n] += (double)s * dx;
+        }
         P.xh[n] = 0.f;
     }
 }
 
 __global__ void k_set_state(pn_state* st, double rr, double beta, double rr_max, double rr_target, double delta2,
-                            int max_iters, int reset_iters) {
+                            int max_iters, int reset_iters, double xskip_min) {
+    st->alpha2 = 0.0;
+    st->beta_prev = 0.0;
+    st->xskip_min = xskip_min;
+    st->xpend = 0;
     st->rr = rr;
     st->rr_old = rr;
     st->beta = beta;
@@ -92,7 +105,7 @@ __global__ void k_set_state(pn_state* st, double rr, double beta, double rr_max,
     st->rr_target = rr_target;
     st->delta2 = delta2;
     st->max_iters = max_iters;
-    if (reset_iters) st->iters = 0;
+    if (reset_iters) { st->iters = 0; st->n_xskip = 0; }
     st->flag = PN_FLAG_RUN;
     st->ticket = 0u;
 }
@@ -152,8 +165,9 @@ cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st,
     return cudaGetLastError();
 }
 cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,
-                                double delta2, int max_iters, int reset_iters, cudaStream_t st, int* launches) {
-    k_set_state<<<1, 1, 0, st>>>(P.st, rr, beta, rr_max, rr_target, delta2, max_iters, reset_iters);
+                                double delta2, int max_iters, int reset_iters, double xskip_min, cudaStream_t st,
+                                int* launches) {
+    k_set_state<<<1, 1, 0, st>>>(P.st, rr, beta, rr_max, rr_target, delta2, max_iters, reset_iters, xskip_min);
     ++*launches;
     return cudaGetLastError();
 }

@@ -551,3 +551,19 @@ def test_graph_replay_is_bit_identical(pn, kernel):
         ref = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 0})
         assert np.array_equal(P, ref[1])
     h.close()
+
+
+@pytest.mark.parametrize("maker,direction,periodic", [
+    (lambda i: i.cfg4_fbm_cut_3d(64, 64, 64), 0, False), (lambda i: i.cfg3_percolation_3d(40, 33, 50), 2, True),
+    (lambda i: i.cfg2_fbm_2d(300, 200), 1, False), (lambda i: i.iid_diluted(17, 9, 5, seed=3, p=0.7), 0, True)])
+def test_deferred_solution_update(pn, oracle, maker, direction, periodic):
+    """PN_OPT_XDEFER: the single-kernel scheme folds two search directions into x_hat every other iteration (the earlier
+    one recovered as (p - r) / beta).  Same parity bar with it on (default) and off, for odd and even iteration counts
+    at the flush (several residual replacements per solve hit both), and a comparable iteration count."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    on, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_XDEFER: 1, pn.PN_OPT_KERNEL: 3}, periodic=periodic)
+    off, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_XDEFER: 0, pn.PN_OPT_KERNEL: 3}, periodic=periodic)
+    assert on.inner_iters <= 1.05 * off.inner_iters + 5
+    for chunk in (1, 5):        # host polls at other iteration parities
+        compare(pn, oracle, net, direction, opts={pn.PN_OPT_CHUNK: chunk, pn.PN_OPT_KERNEL: 3}, periodic=periodic)
