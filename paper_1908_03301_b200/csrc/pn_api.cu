@@ -355,7 +355,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     const int scheme = pn_resolve_variant(g, ctx->variant);
-    const int fused = scheme == 3;
+    const int fused = scheme >= 3;   // one kernel per iteration; r double-buffered by iteration parity
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)

@@ -149,8 +149,8 @@ int grid_for(long long work_items) {
 // 1024^2); 1 = reference two-kernel iteration, 2 = two-kernel iteration with the TMA S4 kernel, 3 = single fused
 // TMA kernel.
 int pn_resolve_variant(const pn_geom& g, int variant) {
-    (void)g;
     if (variant == 0) return pn_tma_supported() ? 3 : 1;
+    if (variant == 4 && !pn_fused2_supported(g)) return 3;   // 2D lattices, periodic faces: the q-storing kernel
     return variant;
 }
 
@@ -162,22 +162,26 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     const int nb = grid_for(nvec);
     pn_tma_plan* plan = nullptr;
     pn_fused_plan* fplan = nullptr;
+    pn_fused2_plan* gplan = nullptr;
     if (scheme == 2 && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) return cudaErrorNotSupported;
     if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
+    if (scheme == 4 && !(pn_tma_supported() && pn_fused2_plan_build(&gplan, g, P))) return cudaErrorNotSupported;
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];   // periodic lateral faces: k_wrap_fix finishes kernel A
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);
     for (int it = 0; it < iterations && e == cudaSuccess; ++it) {
-        if (scheme == 3) e = pn_launch_cg_fused(fplan, g, P, st);
+        if (scheme == 4) e = pn_launch_cg_fused2(gplan, g, P, st);
+        else if (scheme == 3) e = pn_launch_cg_fused(fplan, g, P, st);
         else if (scheme == 2) e = pn_launch_stencil_tma(plan, g, P, st);
         else k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2, wrap ? 1 : 0);
-        if (wrap && e == cudaSuccess) e = pn_launch_wrap_fix(g, P, scheme == 3, st);
+        if (wrap && e == cudaSuccess) e = pn_launch_wrap_fix(g, P, scheme == 3, st);   // (scheme 4 never runs with wrap)
         if (ev) cudaEventRecord(ev[2 * it + 1], st);
-        if (scheme != 3) k_update<<<nb, TPB, 0, st>>>(nvec, P);
+        if (scheme < 3) k_update<<<nb, TPB, 0, st>>>(nvec, P);
         if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
     pn_tma_plan_free(plan);
     pn_fused_plan_free(fplan);
-    *launches += ((scheme == 3 ? 1 : 2) + (wrap ? 1 : 0)) * iterations;
+    pn_fused2_plan_free(gplan);
+    *launches += ((scheme >= 3 ? 1 : 2) + (wrap ? 1 : 0)) * iterations;
     return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -226,6 +226,13 @@ cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const 
 cudaError_t pn_launch_wrap_fix(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st);
 cudaError_t pn_launch_wrap_copy(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 
+// Single-kernel iteration that recomputes q instead of storing it (pn_fused2_tma.cu): 3D, no-flux faces only
+struct pn_fused2_plan;
+bool pn_fused2_supported(const pn_geom& g);
+bool pn_fused2_plan_build(pn_fused2_plan** out, const pn_geom& g, const pn_ptrs& P);
+void pn_fused2_plan_free(pn_fused2_plan* pl);
+cudaError_t pn_launch_cg_fused2(const pn_fused2_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
+
 // Which iteration scheme a PN_OPT_KERNEL value selects on this lattice: 1 = reference two-kernel,
 // 2 = two-kernel with the TMA S4 kernel, 3 = single fused TMA kernel
 int pn_resolve_variant(const pn_geom& g, int variant);

@@ -89,10 +89,10 @@ inline bool make_map(CUtensorMap* m, const pn_geom& g, const float* base_with_ha
 
 // z-chunk length of the 2.5D march: balance the persistent grid against the `extra_bytes_per_chunk_node` every
 // chunk pays for its two extra leading planes (per node of a plane, against `bytes_per_node` of useful traffic)
-inline int choose_lz(int nz, int tiles, int nblocks, double bytes_per_node, double extra_bytes_per_chunk_node) {
+inline int choose_lz(int nz, int tiles, int nblocks, double bytes_per_node, double extra_bytes_per_chunk_node, int max_lz = 64) {
     int best = 1;
     double best_eff = 0.0;
-    for (int lz = 4; lz <= 64; ++lz) {
+    for (int lz = 4; lz <= max_lz; ++lz) {
         const int chunks = (nz + lz - 1) / lz;
         const long long items = (long long)chunks * tiles;
         const long long rounds = (items + nblocks - 1) / nblocks;

@@ -114,7 +114,7 @@ def test_cfg4_sibling_128(pn, oracle):
 @pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 31, 7), (130, 6, 3)])
 @pytest.mark.parametrize("direction", [0, 1, 2])
 @pytest.mark.parametrize("p", [1.0, 0.6])
-@pytest.mark.parametrize("kernel", [1, 2, 3])
+@pytest.mark.parametrize("kernel", [1, 2, 3, 4])
 def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
     """kernel 1 = reference two-kernel iteration, 2 = TMA-fed 2.5D S4 kernel + S5 kernel, 3 = single fused TMA
     kernel per iteration (2 and 3 forced, whatever the size)."""
@@ -133,7 +133,7 @@ def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("kernel", [2, 3])
+@pytest.mark.parametrize("kernel", [2, 3, 4])
 @pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
 def test_tma_kernel_multi_tile(pn, oracle, shape, direction, kernel):
     """Lattices wider than one 256-node TMA box and taller than one 8-row tile: x and y halos between
@@ -151,7 +151,7 @@ def test_tma_kernel_2d_wide(pn, oracle, kernel):
     compare(pn, oracle, net, 1, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("kernel", [1, 2, 3])
+@pytest.mark.parametrize("kernel", [1, 2, 3, 4])
 def test_kernel_variants(pn, oracle, kernel):
     """Both S4 kernels must pass the same parity bar (0 = automatic choice is what the other tests use)."""
     from paper_1908_03301_b200 import inputs
@@ -330,7 +330,7 @@ def test_deterministic(pn):
     """Fixed-order grid reductions: two solves of the same input agree bit for bit."""
     from paper_1908_03301_b200 import inputs
     net = inputs.cfg3_percolation_3d(40, 40, 40)
-    for kernel in (1, 3):
+    for kernel in (1, 3, 4):
         a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel})
         b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel})
         assert a[0].inner_iters == b[0].inner_iters
@@ -567,3 +567,20 @@ def test_deferred_solution_update(pn, oracle, maker, direction, periodic):
     assert on.inner_iters <= 1.05 * off.inner_iters + 5
     for chunk in (1, 5):        # host polls at other iteration parities
         compare(pn, oracle, net, direction, opts={pn.PN_OPT_CHUNK: chunk, pn.PN_OPT_KERNEL: 3}, periodic=periodic)
+
+
+@pytest.mark.parametrize("maker,direction", [
+    (lambda i: i.cfg4_fbm_cut_3d(128, 128, 128), 0), (lambda i: i.cfg3_percolation_3d(64, 64, 64), 1),
+    (lambda i: i.cfg5_stratified_3d(48, 48, 48), 2), (lambda i: i.iid_diluted(515, 19, 37, seed=2, p=0.8), 0)])
+def test_q_recomputing_kernel(pn, oracle, maker, direction):
+    """PN_OPT_KERNEL = 4 (k_cg_fused2_tma: q recomputed on tile + halo instead of stored).  Same parity bar; the
+    iteration count stays that of the q-storing kernel to within a few per cent (same arithmetic up to the rounding of
+    the operator application); x_hat deferral on and off; odd chunk lengths."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    tol = 1e-13 if net.n_nodes >= 2 ** 21 else 1e-12
+    k4, *_ = compare(pn, oracle, net, direction, tol=tol, opts={pn.PN_OPT_KERNEL: 4})
+    k3, *_ = compare(pn, oracle, net, direction, tol=tol, opts={pn.PN_OPT_KERNEL: 3})
+    assert k4.kernel_scheme == 4 and k3.kernel_scheme == 3
+    assert abs(k4.inner_iters - k3.inner_iters) <= 0.10 * k3.inner_iters + 5
+    compare(pn, oracle, net, direction, tol=tol, opts={pn.PN_OPT_KERNEL: 4, pn.PN_OPT_XDEFER: 0, pn.PN_OPT_CHUNK: 7})
