@@ -163,6 +163,12 @@ int pn_set_option(pn_ctx* ctx, int key, double value);
 /* Kernel launches enqueued by this handle since pn_create (bench.py's `gpu_launches`). */
 long long pn_launch_count(const pn_ctx* ctx);
 
+/* Convergence record of the last pn_solve: the true fp64 relative residual ||b - A x||_2 / ||b||_2 at every
+ * evaluation (S8(a) S3), the first entry being that of the initial guess; info->outer_cycles of them (at most
+ * 256 are kept).  Copies min(count, capacity) values to the HOST array `out` and returns the count (>= 0), or
+ * PN_ERR_ARG.  `out` may be NULL when capacity == 0 (query). */
+int pn_residual_history(const pn_ctx* ctx, double* out, int capacity);
+
 /* Release the handle (not the workspace).  NULL is allowed. */
 int pn_destroy(pn_ctx* ctx);
 

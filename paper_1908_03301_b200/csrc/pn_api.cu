@@ -18,6 +18,8 @@
 
 #include "pn_internal.cuh"
 
+#define PN_HISTORY_MAX 256
+
 struct pn_ctx {
     int unx, uny, unz;          // user lattice
     bool is2d;
@@ -46,6 +48,8 @@ struct pn_ctx {
     double delta;
     long long launches;
     double flux[4];
+    double hist[PN_HISTORY_MAX];   // true relative residual at every fp64 residual evaluation of the last solve
+    int hist_n;
     bool flux_valid;
     char err[256];
 };
@@ -236,6 +240,13 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
 
 long long pn_launch_count(const pn_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int pn_residual_history(const pn_ctx* ctx, double* out, int capacity) {
+    if (!ctx || capacity < 0 || (capacity > 0 && !out)) return PN_ERR_ARG;
+    const int n = ctx->hist_n < capacity ? ctx->hist_n : capacity;
+    for (int i = 0; i < n; ++i) out[i] = ctx->hist[i];
+    return ctx->hist_n;
+}
+
 const char* pn_last_error(const pn_ctx* ctx) { return ctx ? ctx->err : ""; }
 
 const char* pn_strerror(int code) {
@@ -402,6 +413,8 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     double rn = sqrt(h->acc[0]);
     double rr_hat = h->acc[1];
     int outer = 1;
+    ctx->hist_n = 0;
+    if (nb > 0.0) ctx->hist[ctx->hist_n++] = rn / nb;
     int status = PN_OK;
     int total_iters = 0;
     double t_stencil = 0.0, t_update = 0.0;
@@ -476,6 +489,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
             if (rc) return rc;
             ++outer;
             rn = sqrt(h->acc[0]);
+            if (ctx->hist_n < PN_HISTORY_MAX) ctx->hist[ctx->hist_n++] = rn / nb;
             rr_hat = h->acc[1];
             if (status == PN_ERR_BREAKDOWN) break;
             if (rn <= tol * nb) break;

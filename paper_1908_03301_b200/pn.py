@@ -30,7 +30,7 @@ CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CL
 # every symbol include/pn.h declares (tests check that the library exports each of them)
 SYMBOLS = ("pn_workspace_bytes", "pn_create", "pn_set_conductances", "pn_solve", "pn_get_pressures",
            "pn_get_classes", "pn_flux", "pn_set_option", "pn_launch_count", "pn_destroy", "pn_strerror",
-           "pn_last_error")
+           "pn_last_error", "pn_residual_history")
 
 
 class PnInfo(ctypes.Structure):
@@ -104,6 +104,8 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.pn_set_option.restype = ctypes.c_int
     lib.pn_launch_count.argtypes = [vp]
     lib.pn_launch_count.restype = ctypes.c_longlong
+    lib.pn_residual_history.argtypes = [vp, dp, ctypes.c_int]
+    lib.pn_residual_history.restype = ctypes.c_int
     lib.pn_destroy.argtypes = [vp]
     lib.pn_destroy.restype = ctypes.c_int
     lib.pn_strerror.argtypes = [ctypes.c_int]
@@ -227,6 +229,15 @@ class Network:
         v = [ctypes.c_double() for _ in range(4)]
         self._check(self._lib.pn_flux(self._h, *[ctypes.byref(x) for x in v]))
         return tuple(x.value for x in v)
+
+    def residual_history(self):
+        """True fp64 relative residuals of the last solve, one per residual evaluation (first = initial guess)."""
+        n = self._lib.pn_residual_history(self._h, None, 0)
+        if n < 0:
+            self._check(n)
+        buf = (ctypes.c_double * max(n, 1))()
+        self._lib.pn_residual_history(self._h, buf, n)
+        return [buf[i] for i in range(n)]
 
     def launch_count(self) -> int:
         return int(self._lib.pn_launch_count(self._h))

@@ -50,14 +50,15 @@ def _plane_fluxes(net, P, direction):
     return out
 
 
-def certify(pn, oracle, net, h, direction, tol):
+def certify(pn, oracle, net, h, direction, tol, periodic=False):
     info = h.solve(direction, tol, accept=(pn.PN_OK,))
     P = h.pressures_host()
     cls = h.classes().cpu().numpy()
     fl = h.flux()
     assert info.rel_residual <= tol
     ref_cls = np.empty((net.nz, net.ny, net.nx), dtype=np.int8)
-    rel, pin_err = oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, P, direction, classes_out=ref_cls)
+    rel, pin_err = oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, P, direction, classes_out=ref_cls,
+                                      periodic=periodic)
     assert np.array_equal(cls, ref_cls), "node classes differ from the oracle's serial BFS"
     assert info.n_solved == int(np.count_nonzero(ref_cls == 2))
     assert pin_err == 0.0
@@ -140,3 +141,19 @@ def test_cfg5_full_512cubed_certificate(pn, oracle):
     assert flx[3] == pytest.approx(arith, rel=0.05)
     assert harm * 0.8 <= flz[3] <= harm * 1.05
     assert flx[3] > flz[3]
+
+
+def test_cfg4_full_512cubed_periodic_certificate(pn, oracle):
+    """The same 512^3 network with the paper's own lateral condition (periodic; PN_OPT_LATERAL = 1): the oracle's
+    PERIODIC operator certifies the residual; its no-flux operator must reject the field."""
+    import torch
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg4_fbm_cut_3d()
+    h = pn.Network(net.nx, net.ny, net.nz)
+    h.set_option(pn.PN_OPT_LATERAL, 1)
+    h.set_conductances(*(torch.from_numpy(g).cuda() for g in (net.gx, net.gy, net.gz)))
+    info, fl, pf = certify(pn, oracle, net, h, 0, 1e-10, periodic=True)
+    P = h.pressures_host()
+    h.close()
+    rel0, _ = oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, P, 0)
+    assert rel0 > 1e-6

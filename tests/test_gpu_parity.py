@@ -584,3 +584,20 @@ def test_q_recomputing_kernel(pn, oracle, maker, direction):
     assert k4.kernel_scheme == 4 and k3.kernel_scheme == 3
     assert abs(k4.inner_iters - k3.inner_iters) <= 0.10 * k3.inner_iters + 5
     compare(pn, oracle, net, direction, tol=tol, opts={pn.PN_OPT_KERNEL: 4, pn.PN_OPT_XDEFER: 0, pn.PN_OPT_CHUNK: 7})
+
+
+def test_residual_history(pn):
+    """pn_residual_history: one true fp64 residual per evaluation, strictly falling from the initial guess to the exit
+    value reported in pn_info (reliable updates: every replacement sees a residual at least ~10x smaller)."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg4_fbm_cut_3d(48, 40, 36)
+    h = pn.Network(net.nx, net.ny, net.nz)
+    assert h.residual_history() == []
+    h.set_conductances(net.gx, net.gy, net.gz)
+    info = h.solve(0, 1e-11)
+    hist = h.residual_history()
+    h.close()
+    assert len(hist) == info.outer_cycles >= 3
+    assert hist[-1] == info.rel_residual <= 1e-11
+    assert all(b < a for a, b in zip(hist, hist[1:]))
+    assert 1e-3 < hist[0] < 10.0
