@@ -157,6 +157,12 @@ int pn_get_classes(pn_ctx* ctx, signed char* out, int pointer_is_device);
  * HOST pointers; any may be NULL.  Needs a finished pn_solve (PN_ERR_STATE otherwise). */
 int pn_flux(pn_ctx* ctx, double* q_in, double* q_out, double* g_eff, double* k_eff);
 
+/* Dissipation estimate of the effective conductance: g_e = sum over ALL bonds of g (P_i - P_j)^2 (dP = 1; the energy
+ * identity Q dP = sum g dP_bond^2 of the balance P:53 with eq.(4)).  Equal to g_eff at the exact solution, and
+ * its error is quadratic in the error of the pressures where g_eff's (boundary fluxes) is linear: a cross-check that
+ * holds to ~1e-12 already at a 1e-10 residual (S8(c) consequence (iv)).  HOST pointer.  Needs a finished pn_solve. */
+int pn_dissipation(pn_ctx* ctx, double* g_e);
+
 /* Tuning knobs (PN_OPT_*).  PN_ERR_ARG on an unknown key or out-of-range value. */
 int pn_set_option(pn_ctx* ctx, int key, double value);
 

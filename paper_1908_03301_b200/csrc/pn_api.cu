@@ -598,4 +598,18 @@ int pn_flux(pn_ctx* ctx, double* q_in, double* q_out, double* g_eff, double* k_e
     return PN_OK;
 }
 
+int pn_dissipation(pn_ctx* ctx, double* g_e) {
+    if (!ctx || !g_e) return PN_ERR_ARG;
+    if (!ctx->have_solution) return PN_ERR_STATE;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    int nl = 0;
+    CK(pn_launch_dissipation(ctx->g, ctx->P, ctx->stream, &nl));
+    ctx->launches += nl;
+    int rc = read_state(ctx);
+    if (rc) return rc;
+    *g_e = ctx->h_state->acc[3];
+    return PN_OK;
+}
+
 }  // extern "C"

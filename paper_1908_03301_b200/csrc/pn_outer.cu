@@ -137,6 +137,40 @@ __global__ void k_flux(pn_geom g, pn_ptrs P) {
     }
 }
 
+// ---- dissipation estimate of the effective conductance:  G_E = sum over all bonds g (dP_bond)^2 / dP^2 ----------
+// (dP = 1; energy identity Q dP = sum g dP_bond^2, P:59-61 with P:53).  Its error is QUADRATIC in the error of the
+// pressures, where the boundary fluxes of S8 are linear (SURVEY.md 8(c) consequence (iv)): at the 1e-10 residual of
+// the timing runs it is good to ~1e-12, the boundary-flux G_eff to a few 1e-9.  acc[3] = G_E.
+__global__ void k_dissipation(pn_geom g, pn_ptrs P) {
+    __shared__ double sm[32];
+    __shared__ double tot[1];
+    double e = 0.0;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const double xc = P.x64[n];
+        const float g0 = P.gs[0][n], g1 = P.gs[1][n], g2 = P.gs[2][n];
+        if (g0 != 0.f) { const double d = P.x64[n + 1] - xc; e += (double)g0 * d * d; }
+        if (g1 != 0.f) { const double d = P.x64[n + g.px] - xc; e += (double)g1 * d * d; }
+        if (g2 != 0.f) { const double d = P.x64[n + g.plane] - xc; e += (double)g2 * d * d; }
+    }
+    for (int b = 0; b < 3; ++b) {   // wrap bonds of periodic lateral faces
+        if (!g.wrap[b]) continue;
+        const long long nf = pn_face_count(g, b), span = pn_wrap_span(g, b);
+        for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+            const float gw = P.gsw[b][f];
+            if (gw == 0.f) continue;
+            const long long lo = b == 0 ? (f % g.ny) * (long long)g.px + (f / g.ny) * g.plane
+                                        : (b == 1 ? (f % g.px) + (f / g.px) * g.plane : f);
+            const double d = P.x64[lo + span] - P.x64[lo];
+            e += (double)gw * d * d;
+        }
+    }
+    e = pn_block_sum(e, sm);
+    const double v[1] = {e};
+    if (pn_grid_sum<1>(v, P.slots, &P.st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) P.st->acc[3] = tot[0];
+    }
+}
+
 // ---- padded -> user layout ----------------------------------------------------------------------
 __global__ void k_export_x(pn_geom g, const double* __restrict__ x64, double* __restrict__ out) {
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.n; n += (long long)gridDim.x * blockDim.x) {
@@ -185,6 +219,11 @@ cudaError_t pn_launch_export_x(const pn_geom& g, const pn_ptrs& P, double* out, 
 cudaError_t pn_launch_export_cls(const pn_geom& g, const pn_ptrs& P, signed char* out, int, cudaStream_t st,
                                  int* launches) {
     k_export_cls<<<grid_for(g.n), TPB, 0, st>>>(g, P.cls, out);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_dissipation(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    k_dissipation<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }

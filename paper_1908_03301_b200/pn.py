@@ -30,7 +30,7 @@ CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CL
 # every symbol include/pn.h declares (tests check that the library exports each of them)
 SYMBOLS = ("pn_workspace_bytes", "pn_create", "pn_set_conductances", "pn_solve", "pn_get_pressures",
            "pn_get_classes", "pn_flux", "pn_set_option", "pn_launch_count", "pn_destroy", "pn_strerror",
-           "pn_last_error", "pn_residual_history")
+           "pn_last_error", "pn_residual_history", "pn_dissipation")
 
 
 class PnInfo(ctypes.Structure):
@@ -104,6 +104,8 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.pn_set_option.restype = ctypes.c_int
     lib.pn_launch_count.argtypes = [vp]
     lib.pn_launch_count.restype = ctypes.c_longlong
+    lib.pn_dissipation.argtypes = [vp, dp]
+    lib.pn_dissipation.restype = ctypes.c_int
     lib.pn_residual_history.argtypes = [vp, dp, ctypes.c_int]
     lib.pn_residual_history.restype = ctypes.c_int
     lib.pn_destroy.argtypes = [vp]
@@ -238,6 +240,12 @@ class Network:
         buf = (ctypes.c_double * max(n, 1))()
         self._lib.pn_residual_history(self._h, buf, n)
         return [buf[i] for i in range(n)]
+
+    def dissipation(self) -> float:
+        """G_E = sum over all bonds g (dP_bond)^2: the effective conductance with an error quadratic in that of P."""
+        v = ctypes.c_double()
+        self._check(self._lib.pn_dissipation(self._h, ctypes.byref(v)))
+        return v.value
 
     def launch_count(self) -> int:
         return int(self._lib.pn_launch_count(self._h))

@@ -627,3 +627,26 @@ def test_option_changes_between_solves_on_one_handle(pn, oracle):
     h.close()
     ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, 0, 1e-13)
     assert np.max(np.abs(P - ref.P)) <= 1e-7          # tol 1e-11 here; the parity bar proper is tested at 1e-12
+
+
+@pytest.mark.parametrize("maker,direction,periodic", [
+    (lambda i: i.cfg3_percolation_3d(64, 64, 64), 0, False), (lambda i: i.cfg4_fbm_cut_3d(64, 64, 64), 2, True),
+    (lambda i: i.cfg2_fbm_2d(256, 256), 0, False)])
+def test_dissipation_estimate_meets_1e9_at_the_timing_tolerance(pn, oracle, maker, direction, periodic):
+    """pn_dissipation: G_E = sum_bonds g dP^2 has an error quadratic in that of the pressures (SURVEY.md 8(c) consequence
+    (iv)), so it meets north_star's 1e-9 on the effective conductance already at tol = 1e-10 -- the tolerance bench.py
+    times -- where the boundary-flux G_eff is only good to a few 1e-9."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    ref = oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, direction, 1e-13, periodic=periodic)
+    h = pn.Network(net.nx, net.ny, net.nz)
+    h.set_option(pn.PN_OPT_LATERAL, 1 if periodic else 0)
+    with pytest.raises(pn.PnError) as e:
+        h.dissipation()
+    assert e.value.code == pn.PN_ERR_STATE
+    h.set_conductances(net.gx, net.gy, net.gz)
+    h.solve(direction, 1e-10)
+    g_e, g_eff = h.dissipation(), h.flux()[2]
+    h.close()
+    assert abs(g_e - ref.g_eff) <= 1e-10 * ref.g_eff
+    assert abs(g_eff - ref.g_eff) <= 1e-7 * ref.g_eff
