@@ -82,7 +82,7 @@ enum {
     PN_OPT_MAX_ITERS = 0,   /* inner-iteration budget per solve            (default 200000)         */
     PN_OPT_DELTA = 1,       /* reliable-update threshold: fp64 residual replacement when the fp32
                                recursive residual has fallen by this factor since the last one
-                               (default 0.1; S8(c) reading 4)                                       */
+                               (default 0.3; S8(c) reading 4)                                       */
     PN_OPT_X0 = 2,          /* initial guess on solved nodes: 0 = zero, 1 = linear profile along the
                                solve axis (default 1; S8(c) reading 6), 2 = warm start: the pressures
                                this handle's previous solve left (S8(f) item 4: re-solves after a
