@@ -90,12 +90,14 @@ enum {
     PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32)            */
     PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
-    PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (3),
+    PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
+                               memory -- at most 7168 padded floats per array, no periodic faces -- else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept for cross-checks and small lattices), 2 = TMA-fed 2.5D S4 kernel
                                + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
                                4 = experimental: one kernel per iteration that recomputes q instead of storing it
-                               (32 B per node, but measured slower than 3; 3D, no-flux faces only, else 3)  */
+                               (32 B per node, but measured slower than 3; 3D, no-flux faces only, else 3),
+                               5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory     */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
     PN_OPT_LATERAL = 8,     /* lateral (side) faces: 0 (default) = no-flux (north_star, configs[0]); 1 = periodic,

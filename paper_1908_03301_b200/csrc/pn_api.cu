@@ -366,7 +366,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     const int scheme = pn_resolve_variant(g, ctx->variant);
-    const int fused = scheme >= 3;   // one kernel per iteration; r double-buffered by iteration parity
+    const int fused = scheme == 3 || scheme == 4;   // one kernel per iteration; r double-buffered by iteration parity
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -447,7 +447,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         // Graph path: whole chunks replayed from one executable graph.  With PN_OPT_PROFILE it is used for the single-kernel
         // scheme only (one kernel per iteration: the chunk's device time / iterations run is that kernel's average launch
         // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
-        const bool graph = ctx->use_graph && ctx->chunk > 1 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme);
+        const bool graph = ctx->use_graph && ctx->chunk > 1 && scheme != 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme);
         const int per_iter = (fused ? 1 : 2) + (any_wrap ? 1 : 0);
         while (true) {
             if (graph) {
@@ -461,6 +461,11 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
             rc = read_state(ctx);
             if (rc) return rc;
             if (ctx->profile && graph) {
+                const int ran = h->iters - iters_seen;
+                float ta = 0.f;
+                cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
+                if (ran > 0) { t_stencil += ta; n_timed += ran; }
+            } else if (ctx->profile && scheme == 5) {   // one launch ran `ran` iterations on chip
                 const int ran = h->iters - iters_seen;
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);

@@ -149,7 +149,8 @@ int grid_for(long long work_items) {
 // 1024^2); 1 = reference two-kernel iteration, 2 = two-kernel iteration with the TMA S4 kernel, 3 = single fused
 // TMA kernel.
 int pn_resolve_variant(const pn_geom& g, int variant) {
-    if (variant == 0) return pn_tma_supported() ? 3 : 1;
+    if (variant == 0) return pn_onchip_supported(g) ? 5 : (pn_tma_supported() ? 3 : 1);
+    if (variant == 5 && !pn_onchip_supported(g)) return pn_tma_supported() ? 3 : 1;   // too large for one SM, or periodic faces
     if (variant == 4 && !pn_fused2_supported(g)) return 3;   // 2D lattices, periodic faces: the q-storing kernel
     return variant;
 }
@@ -166,6 +167,13 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     if (scheme == 2 && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) return cudaErrorNotSupported;
     if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
     if (scheme == 4 && !(pn_tma_supported() && pn_fused2_plan_build(&gplan, g, P))) return cudaErrorNotSupported;
+    if (scheme == 5) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu); `iterations` is not a bound here
+        if (ev) cudaEventRecord(ev[0], st);
+        cudaError_t e5 = pn_launch_cg_onchip(g, P, 1 << 30, st);
+        if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
+        *launches += 1;
+        return e5;
+    }
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];   // periodic lateral faces: k_wrap_fix finishes kernel A
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);

@@ -234,6 +234,10 @@ bool pn_fused2_plan_build(pn_fused2_plan** out, const pn_geom& g, const pn_ptrs&
 void pn_fused2_plan_free(pn_fused2_plan* pl);
 cudaError_t pn_launch_cg_fused2(const pn_fused2_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
 
+// Whole inner loop in one CTA's shared memory (pn_onchip.cu): lattices of at most 7168 padded floats per array
+bool pn_onchip_supported(const pn_geom& g);
+cudaError_t pn_launch_cg_onchip(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st);
+
 // Which iteration scheme a PN_OPT_KERNEL value selects on this lattice: 1 = reference two-kernel,
 // 2 = two-kernel with the TMA S4 kernel, 3 = single fused TMA kernel
 int pn_resolve_variant(const pn_geom& g, int variant);

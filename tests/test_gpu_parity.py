@@ -667,3 +667,44 @@ def test_iteration_count_close_to_fp64_cg(pn, oracle, maker, direction, bound):
     assert info.status == pn.PN_OK and info.rel_residual <= 1e-10
     assert info.inner_iters <= bound * ref.iterations
     assert info.inner_iters >= 0.8 * ref.iterations
+
+
+# ---- lattices that fit one SM's shared memory: the whole inner loop in one launch (pn_onchip.cu, scheme 5) ----
+@pytest.mark.parametrize("maker,direction", [
+    (lambda i: i.cfg1_iid_2d(), 0), (lambda i: i.cfg1_iid_2d(), 1), (lambda i: i.iid_diluted(17, 9, 5, seed=7, p=0.6), 0),
+    (lambda i: i.iid_diluted(5, 17, 9, seed=8, p=1.0), 1), (lambda i: i.iid_diluted(9, 5, 17, seed=9, p=0.6), 2),
+    (lambda i: i.iid_diluted(19, 13, 1, seed=11, p=0.7), 1), (lambda i: i.iid_diluted(64, 3, 1, seed=11, p=1.0), 0),
+    (lambda i: i.cfg3_percolation_3d(16, 16, 16, p=0.4), 0), (lambda i: i.cfg4_fbm_cut_3d(18, 16, 14), 2),
+    (lambda i: i.cfg5_stratified_3d(16, 16, 16), 2)])
+def test_onchip_scheme(pn, oracle, maker, direction):
+    """Scheme 5 is the automatic choice on these sizes; same parity bar, iteration count that of the reference
+    two-kernel scheme to within ~10 % (same arithmetic, other summation order; a replacement more or less)."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    auto, P5, fl5, ref = compare(pn, oracle, net, direction)
+    assert auto.kernel_scheme == 5
+    k1, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 1})
+    assert k1.kernel_scheme == 1
+    assert abs(auto.inner_iters - k1.inner_iters) <= 0.15 * k1.inner_iters + 8
+    # the launch count shows the point: one launch per residual replacement instead of two per iteration
+    _, _, _, _, n5 = gpu_solve(pn, net, direction, 1e-12)
+    _, _, _, _, n1 = gpu_solve(pn, net, direction, 1e-12, opts={pn.PN_OPT_KERNEL: 1})
+    assert n5 < n1
+
+
+def test_onchip_scheme_options(pn, oracle):
+    """Budget, zero start, warm start, peeling and the fall-back for periodic faces / large lattices."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg3_percolation_3d(16, 16, 16, p=0.4)
+    info, *_ = gpu_solve(pn, net, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 10})
+    assert info.status == pn.PN_MAX_ITERS and info.kernel_scheme == 5 and info.inner_iters == 10
+    compare(pn, oracle, net, 0, opts={pn.PN_OPT_X0: 0, pn.PN_OPT_DELTA: 0.01})
+    on, *_ = compare(pn, oracle, net, 0, opts={pn.PN_OPT_PEEL: 1})
+    assert on.n_peeled > 0 and on.kernel_scheme == 5
+    per, *_ = compare(pn, oracle, net, 0, periodic=True)
+    assert per.kernel_scheme == 3                       # periodic faces: TMA kernel + k_wrap_fix
+    big, *_ = compare(pn, oracle, inputs.cfg3_percolation_3d(24, 24, 24, p=0.4), 0, opts={pn.PN_OPT_KERNEL: 5})
+    assert big.kernel_scheme == 3                       # 24^3 does not fit: falls back
+    a = gpu_solve(pn, net, 0, 1e-10)
+    b = gpu_solve(pn, net, 0, 1e-10)
+    assert np.array_equal(a[1], b[1]) and a[0].inner_iters == b[0].inner_iters      # deterministic
