@@ -51,6 +51,28 @@ __device__ __forceinline__ void tma_load_3d(float* dst, const CUtensorMap* map, 
 __device__ __forceinline__ void bar_consumers(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
 
 __device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+// Explicit ld.shared / st.shared.  The tile pointers of the TMA kernels come from a rounded-up dynamic shared-memory
+// base and runtime ring slots, so the compiler cannot prove their address space and emits GENERIC accesses (LD.E / ST.E
+// in SASS) for plain dereferences such as lds4() above.  Measured on one B200, same box (profiles/
+// r01_q_recompute_experiment.md): the explicit form makes k_cg_fused2_tma 11.7 % faster (1.094 -> 0.966 ms per
+// iteration at 512^3) but k_cg_fused_tma 1.6 % SLOWER (0.8997 -> 0.9144 ms; `volatile` pins the order of its loads), so
+// only pn_fused2_tma.cu uses these.  `volatile`: never merged or moved across the mbarrier waits and barriers.
+__device__ __forceinline__ float4 slds4(const float* p) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(smem_u32(p)));
+    return v;
+}
+__device__ __forceinline__ float slds1(const float* p) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(smem_u32(p)));
+    return v;
+}
+__device__ __forceinline__ void ssts4(float* p, const float4& v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(p)), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void ssts1(float* p, float v) {
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(smem_u32(p)), "f"(v) : "memory");
+}
 __device__ __forceinline__ float4 fma4(float a, const float4& x, const float4& y) {
     return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
 }
