@@ -24,7 +24,6 @@ __global__ void __launch_bounds__(TPB, 1) k_cg_onchip(pn_geom g, pn_ptrs P, int 
     extern __shared__ __align__(16) float sh[];
     __shared__ double red[32];
     __shared__ double bc[2];                       // broadcast of a reduced sum
-    __shared__ int s_flag;
     const int halo = (int)g.plane, npad = (int)g.npad, len = npad + 2 * halo;
     float* wx = sh + halo;                          // every array: [halo | npad | halo], index 0 = node 0
     float* wy = wx + len;
@@ -115,7 +114,6 @@ __global__ void __launch_bounds__(TPB, 1) k_cg_onchip(pn_geom g, pn_ptrs P, int 
         st->iters = it;
         st->flag = flag;
     }
-    (void)s_flag;
 }
 
 }  // namespace
