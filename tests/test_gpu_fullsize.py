@@ -157,3 +157,42 @@ def test_cfg4_full_512cubed_periodic_certificate(pn, oracle):
     h.close()
     rel0, _ = oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, P, 0)
     assert rel0 > 1e-6
+
+
+def test_maximum_size_layered_closed_form(pn):
+    """Edge case "maximum size": 20 x 8192 x 8190 = 1.34e9 nodes -- 103 GB of workspace, about what one 180 GB B200 holds
+    beside the inputs and the exported pressures; element offsets beyond 2^30 and byte offsets beyond 4 GB in every
+    array (the library's own limit, 2^31 padded nodes, would need 165 GB).  Noise-free z-layers, pressure drop along the short x axis,
+    ZERO start (a few hundred iterations: the y and z bonds couple the rows on the way although no current crosses
+    them at the solution); the answer has a closed form -- P linear in x on all nodes, G_eff = ny * sum_k c_k / (nx - 1).  Inputs are built on the device
+    (no 16 GB host arrays); the check runs on the device too."""
+    import torch
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 150e9:
+        pytest.skip("needs 150 GB of free device memory")
+    nx, ny, nz = 20, 8192, 8190
+    assert pn.load_library().pn_workspace_bytes(nx, ny, 13110) == 0            # 2^31 padded nodes (+ halo planes) are refused
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    c = (0.2 + 1.8 * torch.rand(nz, generator=gen, device="cuda")).to(torch.float32)
+    e = (0.2 + 1.8 * torch.rand(nz, generator=gen, device="cuda")).to(torch.float32)
+    gx = c.reshape(nz, 1, 1).expand(nz, ny, nx).contiguous()
+    gz = e.reshape(nz, 1, 1).expand(nz, ny, nx).contiguous()
+    h = pn.Network(nx, ny, nz)
+    h.set_option(pn.PN_OPT_X0, 0)
+    h.set_conductances(gx, gx, gz)
+    del gz
+    info = h.solve(0, 1e-12, accept=(pn.PN_OK,))
+    fl = h.flux()
+    assert info.n_solved == (nx - 2) * ny * nz and 0 < info.inner_iters <= 2000
+    expect = ny * float(c.to(torch.float64).sum()) / (nx - 1)
+    assert fl[2] == pytest.approx(expect, rel=1e-10)
+    assert fl[0] == pytest.approx(fl[1], rel=1e-10)
+    del gx
+    P = h.pressures()
+    lin = 1.0 - torch.arange(nx, dtype=torch.float64, device="cuda") / (nx - 1)
+    err = 0.0
+    for k0 in range(0, nz, 1024):                       # in slabs: no second 10 GB temporary
+        err = max(err, float((P[k0:k0 + 1024] - lin).abs().max()))
+    h.close()
+    assert err <= 1e-10
