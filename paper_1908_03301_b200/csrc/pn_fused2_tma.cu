@@ -32,8 +32,9 @@ namespace {
 
 using namespace pn_tma;
 
-struct GC {
-    static constexpr int BOXW = 256, TY = 8;
+template <int TY_, int SG_>
+struct GCfg {
+    static constexpr int BOXW = 256, TY = TY_;
     static constexpr int PR = TY + 4;                      // p_old rows  y0-2 .. y0+TY+1
     static constexpr int RR = TY + 2;                      // r, wx, wz, p_new rows  y0-1 .. y0+TY
     static constexpr int WYR = TY + 3;                     // wy rows  y0-2 .. y0+TY
@@ -41,7 +42,7 @@ struct GC {
     static constexpr int NCONS = 64 * TY;                  // consumer threads: one float4 of an own row each, plus ONE node of the
                                                            // two halo rows (2 x 256 nodes = NCONS) for step A
     static constexpr int NTHREADS = NCONS + 32;            // + one producer warp
-    static constexpr int SP = 4, SG = 3;                   // ring depths
+    static constexpr int SP = 4, SG = SG_;                 // ring depths
     // P slot (floats)
     static constexpr int P_SL = PR * BOXW, P_SR = P_SL + a32(PR * 4), P_FLOATS = P_SR + a32(PR * 4);
     // G slot (floats): r | wx | wz | wy, each main box then left and right sliver
@@ -86,10 +87,9 @@ __device__ __forceinline__ float4 stencil4(const float4& pc, float pl, float pr,
     return q;
 }
 
-template <int DUMMY>
-__global__ void __launch_bounds__(GC::NTHREADS, 1)
+template <class C>
+__global__ void __launch_bounds__(C::NTHREADS, 1)
 k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz) {
-    using C = GC;
     pn_state* st = P.st;
     if (st->flag != PN_FLAG_RUN) return;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -171,8 +171,6 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
         // ================= consumer warps: thread = (own row ra = 1..TY of the 10 p_new rows, float4 c4 of the row) =====
         const int lane = tid & 31;
         const int ra = (tid >> 6) + 1, c4 = tid & 63;
-        // ... and, in step A, the node (hr, hx) of the two halo rows
-        const int hr = tid < C::BOXW ? 0 : C::RR - 1, hx = tid & (C::BOXW - 1);
         const int o10 = ra * C::BOXW + c4 * 4;                 // own float4 in a 10-row box (r, wx, wz)
         const int oP = (ra + 1) * C::BOXW + c4 * 4;            // own float4 in the 12-row p_old box
         const int oY = (ra + 1) * C::BOXW + c4 * 4;            // own forward-y bonds in the 11-row wy box (row above: - BOXW)
@@ -248,8 +246,9 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                         a_rr += (double)dot4(r_nxt, r_nxt);
                     }
                 }
-                {
-                    // one node of a halo row (scalar; same stencil1 as its owner tile runs on it)
+                for (int hn = tid; hn < 2 * C::BOXW; hn += C::NCONS) {
+                    // nodes of the two halo rows (scalar; same stencil1 as their owner tile runs on them)
+                    const int hr = hn < C::BOXW ? 0 : C::RR - 1, hx = hn & (C::BOXW - 1);
                     const int iP = (hr + 1) * C::BOXW + hx, i10 = hr * C::BOXW + hx;
                     const float pc = slds1(Pc + (iP));
                     const float pl = hx == 0 ? slds1(Pc + (C::P_SL + (hr + 1) * 4 + 3)) : slds1(Pc + (iP - 1));
@@ -262,7 +261,7 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                 }
                 if (tid < 2 * C::RR) {
                     // the nodes just left (side 0: column x0-1) and right (side 1: column x0+256) of the tile, 10 rows each
-                    const int side = tid / C::RR, hr = tid - side * C::RR, hp = hr + 1;   // (shadows the halo-row hr)
+                    const int side = tid / C::RR, hr = tid - side * C::RR, hp = hr + 1;
                     const int ps = side ? C::P_SR + hp * 4 : C::P_SL + hp * 4 + 3;        // the node in a p_old sliver
                     const int gs = side ? C::V10_SR + hr * 4 : C::V10_SL + hr * 4 + 3;    // ... in a 10-row sliver
                     const int ys = side ? C::WY_SR + hp * 4 : C::WY_SL + hp * 4 + 3;      // ... in the wy sliver (own row)
@@ -331,8 +330,8 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
     }
 }
 
+template <class C>
 bool build_gmaps(pn_gmaps* M, const pn_geom& g, const pn_ptrs& P) {
-    using C = GC;
     const long long h = g.plane;
     const float* pv[2] = {P.p, P.p2};
     const float* rv[2] = {P.r, P.r2};
@@ -354,6 +353,11 @@ bool build_gmaps(pn_gmaps* M, const pn_geom& g, const pn_ptrs& P) {
 
 }  // namespace
 
+// 256 x 8 tile, G ring of 3: the loads lead the march by one plane.  GCfg<6, 4> (256 x 6 tile, G ring of 4, a lead of two
+// planes, 127 registers) was measured too: 0.9651 vs 0.9665 ms per iteration at 512^3 -- no difference, the kernel is not
+// waiting for a longer lead (profiles/r01_q_recompute_experiment.md).
+typedef GCfg<8, 3> GC8;
+
 struct pn_fused2_plan {
     pn_gmaps maps;
 };
@@ -365,18 +369,18 @@ bool pn_fused2_plan_build(pn_fused2_plan** out, const pn_geom& g, const pn_ptrs&
     if (!get_encoder() || !pn_fused2_supported(g)) return false;
     pn_fused2_plan* pl = new (std::nothrow) pn_fused2_plan;
     if (!pl) return false;
-    if (!build_gmaps(&pl->maps, g, P)) { delete pl; return false; }
+    if (!build_gmaps<GC8>(&pl->maps, g, P)) { delete pl; return false; }
     *out = pl;
     return true;
 }
 
 void pn_fused2_plan_free(pn_fused2_plan* pl) { delete pl; }
 
-cudaError_t pn_launch_cg_fused2(const pn_fused2_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st) {
-    using C = GC;
+template <class C>
+static cudaError_t launch_fused2(const pn_fused2_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st) {
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_cg_fused2_tma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(k_cg_fused2_tma<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
@@ -387,6 +391,10 @@ cudaError_t pn_launch_cg_fused2(const pn_fused2_plan* pl, const pn_geom& g, cons
     const int nchunks = (g.nz + lz - 1) / lz;
     const long long total = (long long)ntx * nty * nchunks;
     const int nb = (int)(total < sms ? total : sms);
-    k_cg_fused2_tma<0><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(pl->maps, g, P, ntx, nty, nchunks, lz);
+    k_cg_fused2_tma<C><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(pl->maps, g, P, ntx, nty, nchunks, lz);
     return cudaGetLastError();
+}
+
+cudaError_t pn_launch_cg_fused2(const pn_fused2_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st) {
+    return launch_fused2<GC8>(pl, g, P, st);
 }
