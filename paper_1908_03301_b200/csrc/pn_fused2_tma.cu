@@ -274,8 +274,9 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                     const float rn = fmaf(nal, q, slds1(Gc + (C::R_ + gs)));
                     ssts1(ringA + hr * C::W + (side ? 4 + C::BOXW : 3), fmaf(beta, pc, rn));
                 }
-                bar_consumers(C::NCONS);
-                // ---- step C: q_t on plane c = a-1 from the p_new ring; weights of plane c from G(a-1) ----
+                // ---- step C: q_t on plane c = a-1; weights of plane c from G(a-1).  It reads, besides this thread's own
+                // registers, only rows of ring plane a-1, complete since the barrier that ended the previous step: no
+                // barrier between A and C, the two operator applications of a step are independent instruction streams ----
                 {
                     const int c = a - 1;
                     const float4 gz = slds4(Gm + C::WZ + o10);
@@ -302,6 +303,7 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                 }
                 r_cur = r_nxt;
                 pn_m2 = pn_m1; pn_m1 = pn;
+                bar_consumers(C::NCONS);   // ring plane a complete (rows written by other warps) before the next step's C reads it
                 __syncwarp();
                 if (lane == 0) {
                     mbar_arrive(emptyP + (iP - 1) % C::SP);     // P(a-1)
