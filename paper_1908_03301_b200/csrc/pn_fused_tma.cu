@@ -35,6 +35,10 @@ template <int NBX_, int TY_, bool HAS_Y_, int S_>
 struct FCfg {
     static constexpr int NBX = NBX_, TY = TY_, S = S_;
     static constexpr bool HAS_Y = HAS_Y_;
+    // where the CTA barrier of a plane step sits: at its END (phases A and C become independent instruction streams) or
+    // between the phases.  Measured on one box (profiles/r01_barrier_placement.md): end is 3.6 % faster on the 3D tile
+    // (512^3) and 3.1 % slower on the 2D one (2048^2)
+    static constexpr bool BAR_END = HAS_Y_;
     static constexpr int BOXW = 256;                       // TMA box limit per dimension
     static constexpr int TXW = BOXW * NBX;                 // tile width in nodes
     static constexpr int RH = TY + (HAS_Y ? 2 : 0);        // rows of r, q, p and p_new including the y halo
@@ -223,8 +227,10 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
                     *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + C::TXW : 0)) = fma4(beta, lds4(sg + C::P_ + o), rn);
                 }
-                bar_consumers(C::NCONS);
-                // ---- phase C: q_t(kk) = p_t - W p_t from the ring, weights from the stage ----
+                if (!C::BAR_END) bar_consumers(C::NCONS);
+                // ---- phase C: q_t(kk) = p_t - W p_t from the ring, weights from the stage.  Of plane kk+1, written just above,
+                // it reads only this thread's own float4; everything it reads from other threads belongs to planes kk and kk-1,
+                // complete since the barrier that ended the previous step: no barrier is NEEDED between the phases ----
                 if (kk >= k0) {
                     const float* r0 = ring + ((kk + 4) & 3) * (C::RH * C::W) + rrow * C::W + rcol;
                     const float4 pc = lds4(r0);
@@ -268,6 +274,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     wzm = lds4(sg + C::WZ + own_ty);   // wz(k0-1): the backward z bond of the first plane
                 }
                 r_cur = r_nxt;
+                if (C::BAR_END) bar_consumers(C::NCONS);   // plane kk+1 of the ring complete before the next step's phase C reads its rows
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + s);
             }
