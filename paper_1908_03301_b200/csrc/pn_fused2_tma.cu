@@ -93,7 +93,10 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
     pn_state* st = P.st;
     if (st->flag != PN_FLAG_RUN) return;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    float* pslots = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    // no integer round trip on the base pointer: the compiler then proves the shared address space itself (LDS / STS, free
+    // to schedule); TMA destinations need 128-byte alignment, checked rather than assumed
+    float* pslots = reinterpret_cast<float*>(smem_raw);
+    if ((smem_u32(smem_raw) & 127u) != 0u) __trap();
     float* gslots = pslots + C::SP * C::P_FLOATS;
     float* ring = gslots + C::SG * C::G_FLOATS;
     uint64_t* fullP = reinterpret_cast<uint64_t*>(ring + C::RING_FLOATS);
@@ -193,9 +196,9 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
             mbar_wait(fullP + (itP + 1) % C::SP, ((itP + 1) / C::SP) & 1u);        // P(k0-1)
             mbar_wait(fullG + itG % C::SG, (itG / C::SG) & 1u);                    // G(k0-2): its wz only
             // own float4 of p_old(a-1), p_old(a) and of wz(a-1) rotate through registers from plane to plane
-            float4 pA_m = slds4(pslots + (itP % C::SP) * C::P_FLOATS + oP);
-            float4 pA_c = slds4(pslots + ((itP + 1) % C::SP) * C::P_FLOATS + oP);
-            float4 gA_zm = slds4(gslots + (itG % C::SG) * C::G_FLOATS + C::WZ + o10);
+            float4 pA_m = lds4(pslots + (itP % C::SP) * C::P_FLOATS + oP);
+            float4 pA_c = lds4(pslots + ((itP + 1) % C::SP) * C::P_FLOATS + oP);
+            float4 gA_zm = lds4(gslots + (itG % C::SG) * C::G_FLOATS + C::WZ + o10);
             float4 pn_m1 = make_float4(0.f, 0.f, 0.f, 0.f), pn_m2 = pn_m1;   // own p_new(a-1), p_new(a-2)
             for (int a = k0 - 1; a <= k1; ++a) {
                 const unsigned iP = itP + (unsigned)(a - (k0 - 2)), iG = itG + (unsigned)(a - (k0 - 2));
@@ -216,22 +219,22 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                 float4 r_nxt, pn;
                 {
                     const float4 pc = pA_c;
-                    const float4 pzp = slds4(Pp + oP);
+                    const float4 pzp = lds4(Pp + oP);
                     float pl = __shfl_up_sync(0xffffffffu, pc.w, 1);
                     float pr = __shfl_down_sync(0xffffffffu, pc.x, 1);
-                    if (lane == 0) pl = c4 == 0 ? slds1(Pc + (C::P_SL + (ra + 1) * 4 + 3)) : slds1(Pc + (oP - 1));
-                    if (lane == 31) pr = c4 == 63 ? slds1(Pc + (C::P_SR + (ra + 1) * 4)) : slds1(Pc + (oP + 4));
-                    const float4 gx = slds4(Gc + C::WX + o10);
+                    if (lane == 0) pl = c4 == 0 ? slds1(Pc + (C::P_SL + (ra + 1) * 4 + 3)) : (*(Pc + (oP - 1)));
+                    if (lane == 31) pr = c4 == 63 ? slds1(Pc + (C::P_SR + (ra + 1) * 4)) : (*(Pc + (oP + 4)));
+                    const float4 gx = lds4(Gc + C::WX + o10);
                     float gxl = __shfl_up_sync(0xffffffffu, gx.w, 1);
-                    if (lane == 0) gxl = c4 == 0 ? slds1(Gc + (C::WX + C::V10_SL + ra * 4 + 3)) : slds1(Gc + (C::WX + o10 - 1));
-                    const float4 gz = slds4(Gc + C::WZ + o10);
-                    const float4 q = stencil4(pc, pl, pr, slds4(Pc + oP - C::BOXW), slds4(Pc + oP + C::BOXW), pA_m, pzp,
-                                              gxl, gx, slds4(Gc + C::WY + oY - C::BOXW), slds4(Gc + C::WY + oY), gA_zm, gz);
+                    if (lane == 0) gxl = c4 == 0 ? (*(Gc + (C::WX + C::V10_SL + ra * 4 + 3))) : (*(Gc + (C::WX + o10 - 1)));
+                    const float4 gz = lds4(Gc + C::WZ + o10);
+                    const float4 q = stencil4(pc, pl, pr, lds4(Pc + oP - C::BOXW), lds4(Pc + oP + C::BOXW), pA_m, pzp,
+                                              gxl, gx, lds4(Gc + C::WY + oY - C::BOXW), lds4(Gc + C::WY + oY), gA_zm, gz);
                     pA_m = pc; pA_c = pzp; gA_zm = gz;
-                    const float4 ro = slds4(Gc + C::R_ + o10);       // r_{t-1}
+                    const float4 ro = lds4(Gc + C::R_ + o10);       // r_{t-1}
                     r_nxt = fma4(nal, q, ro);
                     pn = fma4(beta, pc, r_nxt);
-                    ssts4(ringA + oR, pn);
+                    *reinterpret_cast<float4*>(ringA + oR) = (pn);
                     if (inb && own_plane) {
                         const long long n = (long long)a * g.plane + nrow;
                         *reinterpret_cast<float4*>(r_out + n) = r_nxt;
@@ -250,14 +253,14 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                     // nodes of the two halo rows (scalar; same stencil1 as their owner tile runs on them)
                     const int hr = hn < C::BOXW ? 0 : C::RR - 1, hx = hn & (C::BOXW - 1);
                     const int iP = (hr + 1) * C::BOXW + hx, i10 = hr * C::BOXW + hx;
-                    const float pc = slds1(Pc + (iP));
-                    const float pl = hx == 0 ? slds1(Pc + (C::P_SL + (hr + 1) * 4 + 3)) : slds1(Pc + (iP - 1));
-                    const float pr = hx == C::BOXW - 1 ? slds1(Pc + (C::P_SR + (hr + 1) * 4)) : slds1(Pc + (iP + 1));
-                    const float gxl = hx == 0 ? slds1(Gc + (C::WX + C::V10_SL + hr * 4 + 3)) : slds1(Gc + (C::WX + i10 - 1));
-                    const float q = stencil1(pc, pl, pr, slds1(Pc + (iP - C::BOXW)), slds1(Pc + (iP + C::BOXW)), slds1(Pm + (iP)), slds1(Pp + (iP)), gxl, slds1(Gc + (C::WX + i10)),
-                                             slds1(Gc + (C::WY + i10)), slds1(Gc + (C::WY + i10 + C::BOXW)), slds1(Gm + (C::WZ + i10)), slds1(Gc + (C::WZ + i10)));
-                    const float rn = fmaf(nal, q, slds1(Gc + (C::R_ + i10)));
-                    ssts1(ringA + hr * C::W + 4 + hx, fmaf(beta, pc, rn));
+                    const float pc = (*(Pc + (iP)));
+                    const float pl = hx == 0 ? slds1(Pc + (C::P_SL + (hr + 1) * 4 + 3)) : (*(Pc + (iP - 1)));
+                    const float pr = hx == C::BOXW - 1 ? slds1(Pc + (C::P_SR + (hr + 1) * 4)) : (*(Pc + (iP + 1)));
+                    const float gxl = hx == 0 ? (*(Gc + (C::WX + C::V10_SL + hr * 4 + 3))) : (*(Gc + (C::WX + i10 - 1)));
+                    const float q = stencil1(pc, pl, pr, (*(Pc + (iP - C::BOXW))), (*(Pc + (iP + C::BOXW))), (*(Pm + (iP))), (*(Pp + (iP))), gxl, (*(Gc + (C::WX + i10))),
+                                             (*(Gc + (C::WY + i10))), (*(Gc + (C::WY + i10 + C::BOXW))), (*(Gm + (C::WZ + i10))), (*(Gc + (C::WZ + i10))));
+                    const float rn = fmaf(nal, q, (*(Gc + (C::R_ + i10))));
+                    ringA[hr * C::W + 4 + hx] = fmaf(beta, pc, rn);
                 }
                 if (tid < 2 * C::RR) {
                     // the nodes just left (side 0: column x0-1) and right (side 1: column x0+256) of the tile, 10 rows each
@@ -265,34 +268,34 @@ k_cg_fused2_tma(const __grid_constant__ pn_gmaps maps, pn_geom g, pn_ptrs P, int
                     const int ps = side ? C::P_SR + hp * 4 : C::P_SL + hp * 4 + 3;        // the node in a p_old sliver
                     const int gs = side ? C::V10_SR + hr * 4 : C::V10_SL + hr * 4 + 3;    // ... in a 10-row sliver
                     const int ys = side ? C::WY_SR + hp * 4 : C::WY_SL + hp * 4 + 3;      // ... in the wy sliver (own row)
-                    const float pc = slds1(Pc + (ps));
-                    const float pl = side ? slds1(Pc + (hp * C::BOXW + C::BOXW - 1)) : slds1(Pc + (ps - 1));
-                    const float pr = side ? slds1(Pc + (ps + 1)) : slds1(Pc + (hp * C::BOXW));
-                    const float gxl = side ? slds1(Gc + (C::WX + hr * C::BOXW + C::BOXW - 1)) : slds1(Gc + (C::WX + gs - 1));
-                    const float q = stencil1(pc, pl, pr, slds1(Pc + (ps - 4)), slds1(Pc + (ps + 4)), slds1(Pm + (ps)), slds1(Pp + (ps)), gxl, slds1(Gc + (C::WX + gs)),
-                                             slds1(Gc + (C::WY + ys - 4)), slds1(Gc + (C::WY + ys)), slds1(Gm + (C::WZ + gs)), slds1(Gc + (C::WZ + gs)));
-                    const float rn = fmaf(nal, q, slds1(Gc + (C::R_ + gs)));
-                    ssts1(ringA + hr * C::W + (side ? 4 + C::BOXW : 3), fmaf(beta, pc, rn));
+                    const float pc = (*(Pc + (ps)));
+                    const float pl = side ? (*(Pc + (hp * C::BOXW + C::BOXW - 1))) : (*(Pc + (ps - 1)));
+                    const float pr = side ? (*(Pc + (ps + 1))) : (*(Pc + (hp * C::BOXW)));
+                    const float gxl = side ? (*(Gc + (C::WX + hr * C::BOXW + C::BOXW - 1))) : (*(Gc + (C::WX + gs - 1)));
+                    const float q = stencil1(pc, pl, pr, (*(Pc + (ps - 4))), (*(Pc + (ps + 4))), (*(Pm + (ps))), (*(Pp + (ps))), gxl, (*(Gc + (C::WX + gs))),
+                                             (*(Gc + (C::WY + ys - 4))), (*(Gc + (C::WY + ys))), (*(Gm + (C::WZ + gs))), (*(Gc + (C::WZ + gs))));
+                    const float rn = fmaf(nal, q, (*(Gc + (C::R_ + gs))));
+                    ringA[hr * C::W + (side ? 4 + C::BOXW : 3)] = fmaf(beta, pc, rn);
                 }
                 // ---- step C: q_t on plane c = a-1; weights of plane c from G(a-1).  It reads, besides this thread's own
                 // registers, only rows of ring plane a-1, complete since the barrier that ended the previous step: no
                 // barrier between A and C, the two operator applications of a step are independent instruction streams ----
                 {
                     const int c = a - 1;
-                    const float4 gz = slds4(Gm + C::WZ + o10);
+                    const float4 gz = lds4(Gm + C::WZ + o10);
                     if (c >= k0) {
                         const float* r0 = ring + ((c + 4) & 3) * (C::RR * C::W) + oR;
                         const float4 pc = pn_m1;
                         float pl = __shfl_up_sync(0xffffffffu, pc.w, 1);
                         float pr = __shfl_down_sync(0xffffffffu, pc.x, 1);
-                        if (lane == 0) pl = slds1(r0 + (-1));
-                        if (lane == 31) pr = slds1(r0 + (4));
-                        const float4 gx = slds4(Gm + C::WX + o10);
+                        if (lane == 0) pl = (*(r0 + (-1)));
+                        if (lane == 31) pr = (*(r0 + (4)));
+                        const float4 gx = lds4(Gm + C::WX + o10);
                         float gxl = __shfl_up_sync(0xffffffffu, gx.w, 1);
-                        if (lane == 0) gxl = c4 == 0 ? slds1(Gm + (C::WX + C::V10_SL + ra * 4 + 3)) : slds1(Gm + (C::WX + o10 - 1));
-                        const float4 q = stencil4(pc, pl, pr, slds4(r0 - C::W), slds4(r0 + C::W),
+                        if (lane == 0) gxl = c4 == 0 ? (*(Gm + (C::WX + C::V10_SL + ra * 4 + 3))) : (*(Gm + (C::WX + o10 - 1)));
+                        const float4 q = stencil4(pc, pl, pr, lds4(r0 - C::W), lds4(r0 + C::W),
                                                   pn_m2, pn, gxl, gx,
-                                                  slds4(Gm + C::WY + oY - C::BOXW), slds4(Gm + C::WY + oY), wzC, gz);
+                                                  lds4(Gm + C::WY + oY - C::BOXW), lds4(Gm + C::WY + oY), wzC, gz);
                         if (inb) {
                             a_pq += (double)dot4(pc, q);
                             a_rq += (double)dot4(r_cur, q);

@@ -55,8 +55,9 @@ __device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cas
 // base and runtime ring slots, so the compiler cannot prove their address space and emits GENERIC accesses (LD.E / ST.E
 // in SASS) for plain dereferences such as lds4() above.  Measured on one B200, same box (profiles/
 // r01_q_recompute_experiment.md): the explicit form makes k_cg_fused2_tma 11.7 % faster (1.094 -> 0.966 ms per
-// iteration at 512^3) but k_cg_fused_tma 1.6 % SLOWER (0.8997 -> 0.9144 ms; `volatile` pins the order of its loads), so
-// only pn_fused2_tma.cu uses these.  `volatile`: never merged or moved across the mbarrier waits and barriers.
+// iteration at 512^3) but k_cg_fused_tma 1.6 % SLOWER (0.8997 -> 0.9144 ms; `volatile` pins the order of its loads).
+// pn_fused2_tma.cu has since dropped the integer round trip on its base pointer, so the compiler emits LDS itself
+// (another 2.2 %); these helpers are kept for kernels whose pointers cannot be kept in the shared space.  `volatile`: never merged or moved across the mbarrier waits and barriers.
 __device__ __forceinline__ float4 slds4(const float* p) {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(smem_u32(p)));
