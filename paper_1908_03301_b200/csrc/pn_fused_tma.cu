@@ -76,7 +76,13 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     pn_state* st = P.st;
     if (st->flag != PN_FLAG_RUN) return;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    float* stages = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    // The integer round trip on the base pointer makes every tile access a GENERIC load / store (the compiler can no longer
+    // prove the shared address space); without it the compiler emits LDS / STS.  Measured, same box (profiles/
+    // r01_barrier_placement.md): the 3D tile is 5 % FASTER with the generic form (0.8663 vs 0.9127 ms per iteration at 512^3),
+    // the 2D tile 1.2 % faster with LDS (0.03402 vs 0.03447 ms at 2048^2) -- each gets what it measured best with.
+    float* stages = C::HAS_Y ? reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023))
+                             : reinterpret_cast<float*>(smem_raw);
+    if (!C::HAS_Y && (smem_u32(smem_raw) & 127u) != 0u) __trap();   // TMA destinations need 128-byte alignment
     float* ring = stages + C::S * C::STAGE_FLOATS;
     uint64_t* full = reinterpret_cast<uint64_t*>(ring + C::RING_FLOATS);
     uint64_t* empty = full + C::S;
