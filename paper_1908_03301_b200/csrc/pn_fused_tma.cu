@@ -188,7 +188,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
             float4 wzm = make_float4(0.f, 0.f, 0.f, 0.f);
             float4 r_cur = make_float4(0.f, 0.f, 0.f, 0.f);     // r_t on the own float4 of plane kk
             float4 xh_nxt = make_float4(0.f, 0.f, 0.f, 0.f);    // x_hat of plane kk+1, fetched one step ahead
-            if (inb && xmode) xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)k0 * g.plane + nrow);
+            if (inb && xmode) xh_nxt = __ldcs(reinterpret_cast<const float4*>(P.xh + (long long)k0 * g.plane + nrow));
             bar_consumers(C::NCONS);   // the ring is rebuilt per item: nobody may still read the previous item's planes
             for (int kk = k0 - 2; kk < k1; ++kk, ++it) {
                 const int s = it % C::S;
@@ -196,7 +196,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 // x_hat of plane kk+2 goes in flight now and is used one step later
                 const float4 xh_use = xh_nxt;
                 if (inb && xmode && kk + 2 >= k0 + 1 && kk + 2 < k1)
-                    xh_nxt = *reinterpret_cast<const float4*>(P.xh + (long long)(kk + 2) * g.plane + nrow);
+                    xh_nxt = __ldcs(reinterpret_cast<const float4*>(P.xh + (long long)(kk + 2) * g.plane + nrow));
                 mbar_wait(full + s, ph);
                 const float* sg = stages + s * C::STAGE_FLOATS;
                 // ---- phase A: r_t, p_t on plane kk+1 (tile and halo) -> ring; own part -> HBM ----
@@ -210,14 +210,14 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
                     if (kk + 1 >= k0 && kk + 1 < k1 && inb) {
                         const long long n = (long long)(kk + 1) * g.plane + nrow;
-                        *reinterpret_cast<float4*>(r_out + n) = r_nxt;
-                        *reinterpret_cast<float4*>(p_out + n) = pn;
+                        __stcs(reinterpret_cast<float4*>(r_out + n), r_nxt);
+                        __stcs(reinterpret_cast<float4*>(p_out + n), pn);
                         if (xmode) {
                             float4 xn = fma4(al, po, xh_use);
                             if (xmode == 2)
                                 xn = make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
                                                  fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
-                            *reinterpret_cast<float4*>(P.xh + n) = xn;
+                            __stcs(reinterpret_cast<float4*>(P.xh + n), xn);
                         }
                         a_rr += (double)dot4(r_nxt, r_nxt);
                     }
@@ -270,7 +270,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     }
                     q.x = pc.x - q.x; q.y = pc.y - q.y; q.z = pc.z - q.z; q.w = pc.w - q.w;
                     if (inb) {
-                        *reinterpret_cast<float4*>(q_out + (long long)kk * g.plane + nrow) = q;
+                        __stcs(reinterpret_cast<float4*>(q_out + (long long)kk * g.plane + nrow), q);
                         a_pq += (double)dot4(pc, q);
                         a_rq += (double)dot4(r_cur, q);
                         a_qq += (double)dot4(q, q);
