@@ -93,13 +93,20 @@ enum {
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
                                memory -- at most 7168 padded floats per array, no periodic faces -- else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
-                               kernel (kept for cross-checks and small lattices), 2 = TMA-fed 2.5D S4 kernel
+                               kernel (kept as an independently written cross-check), 2 = TMA-fed 2.5D S4 kernel
                                + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
                                4 = experimental: one kernel per iteration that recomputes q instead of storing it
                                (32 B per node, but measured slower than 3; 3D, no-flux faces only, else 3),
                                5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory     */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
+    PN_OPT_PEEL = 7,        /* dead-end peeling: solved nodes left with one open bond carry no current
+                               (S8(c) reading 7, S8(f) item 1); they are removed from the system,
+                               recursively, and take the pressure of the node they hang from after the
+                               solve.  Pressures of all nodes stay those of the full system.
+                               0: never (all solved nodes are unknowns), 1: always, 2 (default): only if
+                               at least 10 % of the solved nodes can be removed (below that -- 3.8 % on
+                               configs[3] -- no gain was measured, and the peeling is undone)       */
     PN_OPT_LATERAL = 8,     /* lateral (side) faces: 0 (default) = no-flux (north_star, configs[0]); 1 = periodic,
                                the paper's own condition ("periodic boundary conditions in the second
                                direction"; S8(f) item 2): every axis other than the solve axis wraps around, and
@@ -108,16 +115,9 @@ enum {
                                not wrap                                                             */
     PN_OPT_GRAPH = 9,       /* 1 (default): a chunk of inner iterations is replayed from a CUDA graph (captured
                                once per geometry / direction / scheme); 0: every kernel launched directly  */
-    PN_OPT_XDEFER = 10,     /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
+    PN_OPT_XDEFER = 10      /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
                                iteration, two search directions at once (the earlier one recovered from p and r):
                                40 instead of 44 bytes per node-iteration on average; 0: every iteration    */
-    PN_OPT_PEEL = 7         /* dead-end peeling: solved nodes left with one open bond carry no current
-                               (S8(c) reading 7, S8(f) item 1); they are removed from the system,
-                               recursively, and take the pressure of the node they hang from after the
-                               solve.  Pressures of all nodes stay those of the full system.
-                               0: never (all solved nodes are unknowns), 1: always, 2 (default): only if
-                               at least 10 % of the solved nodes can be removed (below that the iteration
-                               count does not improve measurably and the peeling is undone)         */
 };
 
 /* Device bytes pn_create needs for an nx x ny x nz lattice (0 on a bad shape). */
