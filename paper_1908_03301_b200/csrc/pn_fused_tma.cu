@@ -36,9 +36,10 @@ struct FCfg {
     static constexpr int NBX = NBX_, TY = TY_, S = S_;
     static constexpr bool HAS_Y = HAS_Y_;
     // where the CTA barrier of a plane step sits: at its END (phases A and C become independent instruction streams) or
-    // between the phases.  Measured on one box (profiles/r01_barrier_placement.md): end is 3.6 % faster on the 3D tile
-    // (512^3) and 3.1 % slower on the 2D one (2048^2)
-    static constexpr bool BAR_END = HAS_Y_;
+    // between the phases.  Measured on one box (profiles/r01_barrier_placement.md): the end is 3.6 % faster on the 3D tile
+    // (512^3); on the 2D tile it was 3.1 % slower with generic shared-memory accesses and is 0.7 % faster now that the 2D
+    // tile uses LDS / STS (see the kernel's first lines)
+    static constexpr bool BAR_END = true;
     static constexpr int BOXW = 256;                       // TMA box limit per dimension
     static constexpr int TXW = BOXW * NBX;                 // tile width in nodes
     static constexpr int RH = TY + (HAS_Y ? 2 : 0);        // rows of r, q, p and p_new including the y halo
