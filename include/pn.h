@@ -38,7 +38,8 @@ typedef struct pn_ctx pn_ctx; /* opaque handle: one network on one device / stre
 enum {
     PN_OK = 0,
     PN_NO_SPANNING_CLUSTER = 1, /* no cluster joins inlet and outlet: Q = 0, pressures = pin values */
-    PN_MAX_ITERS = 2,           /* iteration budget spent or residual stagnated; best iterate kept  */
+    PN_MAX_ITERS = 2,           /* iteration budget spent or residual stagnated; the LAST iterate is
+                                   kept (pn_info.rel_residual is its true residual)                 */
     PN_ERR_ARG = -1,            /* null pointer, bad shape / direction / tol, axis shorter than 3   */
     PN_ERR_STATE = -2,          /* solve before set_conductances, flux / pressures before solve     */
     PN_ERR_VALUE = -3,          /* negative, NaN or Inf conductance on an in-lattice bond           */
@@ -61,7 +62,7 @@ typedef struct {
     int status;            /* the code pn_solve returned                                            */
     int outer_cycles;      /* fp64 true-residual evaluations  r = b - A x  (S8(a) S3)                */
     int inner_iters;       /* fp32 CG iterations (S8(a) S4+S5), summed over the solve               */
-    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 2 or 3) */
+    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3 or 5) */
     double rel_residual;   /* true fp64 ||b - A x||_2 / ||b||_2 over the solved nodes at exit       */
     double b_norm;         /* ||b||_2 of the zero-initial-guess system (S8(c) reading 5)            */
     long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
@@ -93,11 +94,10 @@ enum {
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
                                memory -- at most 7168 padded floats per array, no periodic faces -- else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
-                               kernel (kept as an independently written cross-check), 2 = TMA-fed 2.5D S4 kernel
-                               + S5 kernel, 3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
-                               4 = experimental: one kernel per iteration that recomputes q instead of storing it
-                               (32 B per node, but measured slower than 3; 3D, no-flux faces only, else 3),
-                               5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory     */
+                               kernel (kept as an independently written cross-check),
+                               3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
+                               5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory.
+                               (2 and 4 were round-1 experiments, since removed: PN_ERR_ARG)                   */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
     PN_OPT_PEEL = 7,        /* dead-end peeling: solved nodes left with one open bond carry no current

@@ -24,7 +24,7 @@ class _Info(ctypes.Structure):
                 ("rel_residual", ctypes.c_double), ("q_in", ctypes.c_double),
                 ("q_out", ctypes.c_double), ("g_eff", ctypes.c_double), ("k_eff", ctypes.c_double),
                 ("t_label", ctypes.c_double), ("t_assemble", ctypes.c_double),
-                ("t_pcg", ctypes.c_double)]
+                ("t_pcg", ctypes.c_double), ("it_decade", ctypes.c_int * 16)]
 
 
 @dataclass
@@ -48,6 +48,7 @@ class COracleResult:
     t_assemble: float
     t_pcg: float
     nnz: int
+    it_decade: tuple = ()      # first iteration with recursive ||r||/||b|| <= 1e-k, k = 0..15 (-1: never)
 
 
 def build(force: bool = False) -> str:
@@ -70,6 +71,10 @@ def _load():
                                                         ctypes.POINTER(ctypes.c_byte),
                                                         ctypes.POINTER(_Info)]
         _lib.pno_solve.restype = ctypes.c_int
+        _lib.pno_solve_from.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                                             ctypes.c_int, ctypes.c_int, dp, dp,
+                                                             ctypes.POINTER(ctypes.c_byte), ctypes.POINTER(_Info)]
+        _lib.pno_solve_from.restype = ctypes.c_int
         _lib.pno_certificate.argtypes = [ctypes.c_int] * 3 + [fp, fp, fp, ctypes.c_int, ctypes.c_int, dp, dp, dp,
                                          ctypes.POINTER(ctypes.c_byte)]
         _lib.pno_certificate.restype = ctypes.c_int
@@ -91,21 +96,27 @@ def _prep(nx, ny, nz, g):
 _STATUS = {0: "ok", 1: "no_spanning_cluster", 2: "max_iters"}
 
 
-def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, threads=0, periodic=False):
+def solve(nx, ny, nz, gx, gy, gz, direction=0, tol=1e-13, max_iter=200000, threads=0, periodic=False,
+          P_start=None):
+    """`P_start` (optional, N doubles): starting iterate on the solved nodes instead of the zero start."""
     lib = _load()
     gx, gy, gz = (_prep(nx, ny, nz, g) for g in (gx, gy, gz))
     P = np.empty((nz, ny, nx), dtype=np.float64)
     cls = np.empty((nz, ny, nx), dtype=np.int8)
     info = _Info()
-    rc = lib.pno_solve(nx, ny, nz, _ptr(gx, ctypes.c_float), _ptr(gy, ctypes.c_float),
-                       _ptr(gz, ctypes.c_float), direction, 1 if periodic else 0, tol, max_iter, threads,
-                       _ptr(P, ctypes.c_double), _ptr(cls, ctypes.c_byte), ctypes.byref(info))
+    if P_start is not None:
+        P_start = np.ascontiguousarray(P_start, dtype=np.float64)
+        assert P_start.size == nx * ny * nz
+    rc = lib.pno_solve_from(nx, ny, nz, _ptr(gx, ctypes.c_float), _ptr(gy, ctypes.c_float),
+                            _ptr(gz, ctypes.c_float), direction, 1 if periodic else 0, tol, max_iter, threads,
+                            _ptr(P_start, ctypes.c_double), _ptr(P, ctypes.c_double), _ptr(cls, ctypes.c_byte),
+                            ctypes.byref(info))
     if rc < 0:
         raise ValueError(f"pno_solve failed with code {rc}")
     return COracleResult(P, cls, info.q_in, info.q_out, info.g_eff, info.k_eff, info.iterations,
                          info.restarts, info.rel_residual, info.n_solved, info.n_inlet_only,
                          info.n_outlet_only, info.n_floating, _STATUS[rc], info.threads,
-                         info.t_label, info.t_assemble, info.t_pcg, info.nnz)
+                         info.t_label, info.t_assemble, info.t_pcg, info.nnz, tuple(info.it_decade))
 
 
 def certificate(nx, ny, nz, gx, gy, gz, P, direction=0, classes_out=None, periodic=False):

@@ -36,6 +36,7 @@ typedef struct {
     int threads;
     double rel_residual, q_in, q_out, g_eff, k_eff;
     double t_label, t_assemble, t_pcg;
+    int it_decade[16]; /* record only: first iteration at which the recursive ||r||2/||b||2 <= 1e-k (k = index), -1 if never */
 } pno_info;
 
 static double now(void) {
@@ -222,7 +223,8 @@ static void axpy(long long m, double alpha, const double *x, double *y) {
 
 /* ---- S8c step 5: textbook Jacobi-PCG ---------------------------------------------------------- */
 /* x: start and result.  Stops when the recursive residual 2-norm <= target.  Returns iterations. */
-static int pcg(const csr *A, double *x, double target, int max_iter, double *r, double *z, double *p, double *q) {
+static int pcg(const csr *A, double *x, double target, int max_iter, double *r, double *z, double *p, double *q,
+               double nb, int it_base, int *it_decade) {
     const long long m = A->m;
     int it = 0;
     spmv(A, x, q);
@@ -238,7 +240,10 @@ static int pcg(const csr *A, double *x, double target, int max_iter, double *r, 
         axpy(m, alpha, p, x);
         axpy(m, -alpha, q, r);
         ++it;
-        if (sqrt(dot(m, r, r)) <= target) break;
+        const double rn = sqrt(dot(m, r, r));
+        for (int k = 0; k < 16; ++k) /* record only (tests/golden/make_digest.py): no effect on the iteration */
+            if (it_decade[k] < 0 && rn <= pow(10.0, -k) * nb) it_decade[k] = it_base + it;
+        if (rn <= target) break;
 #pragma omp parallel for schedule(static)
         for (long long u = 0; u < m; ++u) z[u] = r[u] / A->diag[u];
         double rho_new = dot(m, r, z);
@@ -296,13 +301,18 @@ static int setup(lattice *L, int nx, int ny, int nz, const float *gx, const floa
 }
 
 /* Whole path.  P_out: N doubles.  classes_out: N bytes or NULL.  max_threads <= 0: all cores.
+ * P_start: NULL = the textbook zero start (S8c step 5); else N doubles whose values on the solved nodes are the
+ * starting iterate (used by tests/golden/make_digest.py to carry a converged tol-1e-12 solution on to the fp64 floor
+ * without repeating its iterations; same loop, same restarts, only x0 differs).
  * Returns 0 ok / 1 no spanning cluster / 2 max iterations / <0 error. */
-int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction, int periodic,
-              double tol, int max_iter, int max_threads, double *P_out, signed char *classes_out, pno_info *info) {
+int pno_solve_from(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction,
+                   int periodic, double tol, int max_iter, int max_threads, const double *P_start, double *P_out,
+                   signed char *classes_out, pno_info *info) {
     lattice L;
     pno_info local;
     if (!info) info = &local;
     memset(info, 0, sizeof(*info));
+    for (int k = 0; k < 16; ++k) info->it_decade[k] = -1;
     int rc = setup(&L, nx, ny, nz, gx, gy, gz, direction, periodic);
     if (rc) return rc;
 #ifdef _OPENMP
@@ -334,13 +344,15 @@ int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const fl
     double *w = (double *)malloc(sizeof(double) * (size_t)m * 4);
     double *best = (double *)malloc(sizeof(double) * (size_t)m);
     if (!x || !w || !best) return -3;
+    if (P_start) for (long long u = 0; u < m; ++u) x[u] = P_start[A.idx[u]];
     double nb = sqrt(dot(m, A.b, A.b));
     t0 = now();
     double best_rel = INFINITY, rel = 0.0;
     int total = 0, restarts = 0;
     if (nb > 0.0) {
         for (restarts = 0; restarts < 20; ++restarts) {
-            int it = pcg(&A, x, (restarts ? 0.7 : 1.0) * tol * nb, max_iter - total, w, w + m, w + 2 * m, w + 3 * m);
+            int it = pcg(&A, x, (restarts ? 0.7 : 1.0) * tol * nb, max_iter - total, w, w + m, w + 2 * m, w + 3 * m, nb,
+                         total, info->it_decade);
             total += it;
             rel = true_rel_residual(&A, x, w, nb);
             if (rel < best_rel) { best_rel = rel; memcpy(best, x, sizeof(double) * (size_t)m); }
@@ -358,6 +370,12 @@ int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const fl
     csr_free(&A);
     if (!classes_out) free(cls);
     return info->status;
+}
+
+int pno_solve(int nx, int ny, int nz, const float *gx, const float *gy, const float *gz, int direction, int periodic,
+              double tol, int max_iter, int max_threads, double *P_out, signed char *classes_out, pno_info *info) {
+    return pno_solve_from(nx, ny, nz, gx, gy, gz, direction, periodic, tol, max_iter, max_threads, NULL, P_out,
+                          classes_out, info);
 }
 
 /* Independent residual certificate of ANY pressure field (S8c last pin row): ||b - A P_S||2/||b||2 with

@@ -58,8 +58,6 @@ namespace {
 
 constexpr double PN_PEEL_MIN_FRACTION = 0.10;
 
-int g_sm_count = 0;
-
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct layout {
@@ -82,6 +80,7 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     g.n = (long long)nx * ny * nz;
     g.dir = 0; g.n_a = nx; g.stride_a = 1;
     g.wrap[0] = g.wrap[1] = g.wrap[2] = 0;
+    g.sms = 0;
     if (g.npad + 2 * g.plane >= (1ll << 31)) return false;
     L->halo = (size_t)g.plane;
     const size_t vec = (size_t)g.npad + 2 * L->halo;   // elements of a padded array with its two halo planes
@@ -131,8 +130,6 @@ int fail_cuda(pn_ctx* c, cudaError_t e, const char* where) {
 
 }  // namespace
 
-int pn_sm_count() { return g_sm_count > 0 ? g_sm_count : 148; }
-
 extern "C" {
 
 size_t pn_workspace_bytes(int nx, int ny, int nz) {
@@ -165,8 +162,10 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1;
     ctx->delta = 0.3;   // measured: 0.3 needs 11 % fewer iterations than 0.1 on CFG2 2048^2 and the same on CFG3/4/5
     ctx->last_dir_user = -1;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) g_sm_count = prop.multiProcessorCount;
+    // per-handle device facts (no process-global state: handles on different devices are independent)
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms < 1) sms = 148;
+    ctx->g.sms = sms;
     const size_t h = L.halo;
     pn_ptrs& P = ctx->P;
     for (int b = 0; b < 3; ++b) {
@@ -192,6 +191,9 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     P.st = (pn_state*)(ctx->ws + L.off_state);
     P.scratch = (void*)(ctx->ws + L.off_p);   // p and p2 are adjacent: 8 bytes per padded node
     cudaError_t e = cudaMemsetAsync(ctx->ws, 0, L.total, ctx->stream);
+    // large dynamic shared memory is opted into per DEVICE (the attribute is not per process)
+    if (e == cudaSuccess && pn_tma_supported()) e = pn_fused_init_device();
+    if (e == cudaSuccess) e = pn_onchip_init_device();
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_state, sizeof(pn_state));
     for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&ctx->ev[i]);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
@@ -228,7 +230,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_X0: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
         case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
-        case PN_OPT_KERNEL: if (value < 0 || value > 8) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
+        case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
@@ -294,6 +296,13 @@ int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const flo
     return PN_OK;
 }
 
+// field-by-field (a memcmp would also compare padding bytes and force needless re-captures)
+static bool same_geom(const pn_geom& a, const pn_geom& b) {
+    return a.nx == b.nx && a.ny == b.ny && a.nz == b.nz && a.px == b.px && a.plane == b.plane && a.npad == b.npad &&
+           a.n == b.n && a.dir == b.dir && a.n_a == b.n_a && a.stride_a == b.stride_a && a.wrap[0] == b.wrap[0] &&
+           a.wrap[1] == b.wrap[1] && a.wrap[2] == b.wrap[2] && a.sms == b.sms;
+}
+
 static int read_state(pn_ctx* ctx) {
     CK(cudaMemcpyAsync(ctx->h_state, ctx->P.st, sizeof(pn_state), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
@@ -307,7 +316,7 @@ static int read_state(pn_ctx* ctx) {
 // there.  Returns false (graph_exec == nullptr) when capture is unavailable: the caller launches directly.
 static bool ensure_graph(pn_ctx* ctx, int scheme) {
     if (ctx->graph_exec && ctx->graph_scheme == scheme && ctx->graph_chunk == ctx->chunk &&
-        memcmp(&ctx->graph_g, &ctx->g, sizeof(pn_geom)) == 0)
+        same_geom(ctx->graph_g, ctx->g))
         return true;
     if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
     if (!ctx->cap_stream && cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -335,7 +344,8 @@ static bool ensure_graph(pn_ctx* ctx, int scheme) {
     return true;
 }
 
-int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
+// `nl` counts the kernel launches enqueued, whatever the outcome (pn_solve adds it to the handle's total on every return path)
+static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int& nl) {
     if (info) memset(info, 0, sizeof(*info));
     if (!ctx) return PN_ERR_ARG;
     if (direction < 0 || direction > 2 || !(tol > 0.0 && tol < 1.0)) return PN_ERR_ARG;
@@ -357,7 +367,6 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     for (int b = 0; b < 3; ++b) { g.wrap[b] = (ctx->lateral == 1 && b != g.dir && idims[b] >= 2) ? 1 : 0; any_wrap |= g.wrap[b] != 0; }
     const pn_ptrs& P = ctx->P;
     cudaStream_t s = ctx->stream;
-    int nl = 0;
     int rc = PN_OK;
 
     // ---- S1 + set-up ----
@@ -366,7 +375,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     const int scheme = pn_resolve_variant(g, ctx->variant);
-    const int fused = scheme == 3 || scheme == 4;   // one kernel per iteration; r double-buffered by iteration parity
+    const int fused = scheme == 3;   // one kernel per iteration; r double-buffered by iteration parity
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -374,7 +383,7 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         CK(pn_launch_wrap_copy(g, P, s, &nl));
         rc = read_state(ctx);
         if (rc) return rc;
-        if (ctx->h_state->bad_value) { ctx->launches += nl; return PN_ERR_VALUE; }
+        if (ctx->h_state->bad_value) return PN_ERR_VALUE;
         any_closed |= ctx->h_state->any_closed;
     }
     const bool do_label = !ctx->skip_label && any_closed;
@@ -422,10 +431,11 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     if (ctx->profile && ctx->pev_n < 2 * ctx->chunk + 1) {
         for (int i = 0; i < ctx->pev_n; ++i) cudaEventDestroy(ctx->pev[i]);
         delete[] ctx->pev;
-        ctx->pev_n = 2 * ctx->chunk + 1;
-        ctx->pev = new (std::nothrow) cudaEvent_t[ctx->pev_n];
-        if (!ctx->pev) { ctx->pev_n = 0; return PN_ERR_ARG; }
-        for (int i = 0; i < ctx->pev_n; ++i) CK(cudaEventCreate(&ctx->pev[i]));
+        ctx->pev_n = 0;   // counts the events that exist: pn_destroy never sees one that was not created
+        const int want = 2 * ctx->chunk + 1;
+        ctx->pev = new (std::nothrow) cudaEvent_t[want];
+        if (!ctx->pev) return fail_cuda(ctx, cudaErrorMemoryAllocation, "event pool of PN_OPT_PROFILE");
+        for (int i = 0; i < want; ++i) { CK(cudaEventCreate(&ctx->pev[i])); ctx->pev_n = i + 1; }
     }
 
     if (n_solved == 0 || !(nb > 0.0)) {
@@ -510,7 +520,6 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
     if (n_peeled > 0) CK(pn_launch_backfill(g, P, s, &nl));   // dangling ends take the pressure of the node they hang from
     CK(cudaEventRecord(ctx->ev[2], s));
     CK(cudaStreamSynchronize(s));
-    ctx->launches += nl;
     ctx->have_solution = true;
     ctx->ever_solved = true;
     ctx->last_dir_user = direction;
@@ -535,6 +544,13 @@ int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
         info->n_timed_iters = n_timed;
     }
     return status;
+}
+
+int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {
+    int nl = 0;
+    const int rc = solve_impl(ctx, direction, tol, info, nl);
+    if (ctx) ctx->launches += nl;
+    return rc;
 }
 
 int pn_get_pressures(pn_ctx* ctx, double* out, int pointer_is_device) {

@@ -322,14 +322,8 @@ bool build_maps(pn_fmaps* M, const pn_geom& g, const pn_ptrs& P) {
 
 template <class C>
 cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
     const int ntx = (g.px + C::TXW - 1) / C::TXW, nty = (g.ny + C::TY - 1) / C::TY;
-    const int sms = pn_sm_count();
+    const int sms = g.sms;
     const int lz = choose_lz(g.nz, ntx * nty, sms, 44.0, 24.0);   // two extra planes of r, q, p per chunk
     const int nchunks = (g.nz + lz - 1) / lz;
     const long long total = (long long)ntx * nty * nchunks;
@@ -342,6 +336,15 @@ typedef FCfg<1, 8, true, 3> FCfg3D;    // 256 x 8 tile, y halo, 3 stages
 typedef FCfg<8, 1, false, 4> FCfg2D;   // 2048 x 1 tile (lattices held as nx x 1 x ny), 4 stages
 
 }  // namespace
+
+bool pn_tma_supported() { return get_encoder() != nullptr; }
+
+// cudaFuncSetAttribute is per device: pn_create calls this with the handle's device current
+cudaError_t pn_fused_init_device() {
+    cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
+}
 
 struct pn_fused_plan {
     pn_fmaps maps;

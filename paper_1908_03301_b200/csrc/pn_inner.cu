@@ -133,9 +133,9 @@ __global__ void __launch_bounds__(TPB) k_update(int nvec, pn_ptrs P) {
     }
 }
 
-int grid_for(long long work_items) {
+int grid_for(long long work_items, int sms) {
     long long nb = (work_items + TPB - 1) / TPB;
-    long long cap = (long long)pn_sm_count() * 8;
+    long long cap = (long long)sms * 8;
     if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
     if (nb > cap) nb = cap;
     if (nb < 1) nb = 1;
@@ -144,29 +144,25 @@ int grid_for(long long work_items) {
 
 }  // namespace
 
-// PN_OPT_KERNEL: 0 = automatic: the single fused TMA kernel at every size (measured on B200 with graph replay it is
-// at least as fast as the reference pair from 64^2 up: 8.6 vs 9.9 ms at 64^2, 13.9 vs 26.8 ms at 64^3, 113 vs 180 ms at
-// 1024^2); 1 = reference two-kernel iteration, 2 = two-kernel iteration with the TMA S4 kernel, 3 = single fused
-// TMA kernel.
+// PN_OPT_KERNEL: 0 = automatic: the whole loop in one CTA when the lattice fits one SM's shared memory (5), else the
+// single fused TMA kernel at every size (3; measured on B200 with graph replay it is at least as fast as the reference
+// pair from 64^2 up, profiles/r01_small_lattices.md); 1 = reference two-kernel iteration (independently written
+// cross-check).  The two superseded schemes of round 1 (2: TMA S4 kernel + S5 kernel, 4: q recomputed) are gone;
+// their write-ups remain in profiles/r01_tma_kernel.md and profiles/r01_q_recompute_experiment.md.
 int pn_resolve_variant(const pn_geom& g, int variant) {
     if (variant == 0) return pn_onchip_supported(g) ? 5 : (pn_tma_supported() ? 3 : 1);
     if (variant == 5 && !pn_onchip_supported(g)) return pn_tma_supported() ? 3 : 1;   // too large for one SM, or periodic faces
-    if (variant == 4 && !pn_fused2_supported(g)) return 3;   // 2D lattices, periodic faces: the q-storing kernel
     return variant;
 }
 
-// `scheme` is a resolved variant (1, 2 or 3).  ev (optional, 2*iterations+1 events): kernel boundaries, for
+// `scheme` is a resolved variant (1, 3 or 5).  ev (optional, 2*iterations+1 events): kernel boundaries, for
 // the per-kernel timing of PN_OPT_PROFILE (scheme 3: the second interval of every iteration is empty).
 cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int scheme, cudaStream_t st,
                             int* launches, cudaEvent_t* ev) {
     const int nvec = (int)(g.npad / 4);
-    const int nb = grid_for(nvec);
-    pn_tma_plan* plan = nullptr;
+    const int nb = grid_for(nvec, g.sms);
     pn_fused_plan* fplan = nullptr;
-    pn_fused2_plan* gplan = nullptr;
-    if (scheme == 2 && !(pn_tma_supported() && pn_tma_plan_build(&plan, g, P))) return cudaErrorNotSupported;
     if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
-    if (scheme == 4 && !(pn_tma_supported() && pn_fused2_plan_build(&gplan, g, P))) return cudaErrorNotSupported;
     if (scheme == 5) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu); `iterations` is not a bound here
         if (ev) cudaEventRecord(ev[0], st);
         cudaError_t e5 = pn_launch_cg_onchip(g, P, 1 << 30, st);
@@ -178,18 +174,14 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);
     for (int it = 0; it < iterations && e == cudaSuccess; ++it) {
-        if (scheme == 4) e = pn_launch_cg_fused2(gplan, g, P, st);
-        else if (scheme == 3) e = pn_launch_cg_fused(fplan, g, P, st);
-        else if (scheme == 2) e = pn_launch_stencil_tma(plan, g, P, st);
+        if (scheme == 3) e = pn_launch_cg_fused(fplan, g, P, st);
         else k_stencil_simple<<<nb, TPB, 0, st>>>(nvec, g.px, (int)g.plane, P, P.p, P.p2, wrap ? 1 : 0);
-        if (wrap && e == cudaSuccess) e = pn_launch_wrap_fix(g, P, scheme == 3, st);   // (scheme 4 never runs with wrap)
+        if (wrap && e == cudaSuccess) e = pn_launch_wrap_fix(g, P, scheme == 3, st);
         if (ev) cudaEventRecord(ev[2 * it + 1], st);
         if (scheme < 3) k_update<<<nb, TPB, 0, st>>>(nvec, P);
         if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
-    pn_tma_plan_free(plan);
     pn_fused_plan_free(fplan);
-    pn_fused2_plan_free(gplan);
     *launches += ((scheme >= 3 ? 1 : 2) + (wrap ? 1 : 0)) * iterations;
     return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -31,6 +31,7 @@ struct pn_geom {
     int n_a;                    // lattice length along dir
     long long stride_a;         // element stride along dir (1, px, plane)
     int wrap[3];                // INTERNAL axis wraps around (periodic lateral faces); never `dir`, never a length-1 axis
+    int sms;                    // SM count of the handle's device (sizes the persistent grids); set by pn_create
 };
 
 // ---- periodic lateral faces: the wrap bonds live in small FACE arrays, not in the lattice-shaped ones ----
@@ -82,6 +83,9 @@ enum { PN_FLAG_RUN = 0, PN_FLAG_CONVERGED = 1, PN_FLAG_UPDATE = 2, PN_FLAG_BREAK
 // Last-block epilogue of kernel A: alpha = rr / (p.Ap); breakdown guards.
 __device__ __forceinline__ void pn_finish_A(pn_state* st, double pq) {
     st->pq = pq;
+    // kernel A has just applied x_hat += alpha_x p_old: nothing is owed any more.  On the normal path finish_B sets
+    // alpha_x again; on the two early exits below k_flush must not add the same direction a second time.
+    st->alpha_x = 0.0;
     if (st->rr == 0.0) st->flag = PN_FLAG_CONVERGED;
     else if (!(pq > 0.0) || isinf(pq)) st->flag = PN_FLAG_BREAKDOWN;
     else st->alpha = st->rr / pq;
@@ -196,8 +200,6 @@ struct pn_ptrs {
     void* scratch;              // export staging (aliases p, p2)
 };
 
-int pn_sm_count();
-
 cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, bool do_peel, int x0_linear,
                             cudaStream_t st, int* launches);
@@ -227,24 +229,16 @@ cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const 
 cudaError_t pn_launch_wrap_fix(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st);
 cudaError_t pn_launch_wrap_copy(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 
-// Single-kernel iteration that recomputes q instead of storing it (pn_fused2_tma.cu): 3D, no-flux faces only
-struct pn_fused2_plan;
-bool pn_fused2_supported(const pn_geom& g);
-bool pn_fused2_plan_build(pn_fused2_plan** out, const pn_geom& g, const pn_ptrs& P);
-void pn_fused2_plan_free(pn_fused2_plan* pl);
-cudaError_t pn_launch_cg_fused2(const pn_fused2_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
-
 // Whole inner loop in one CTA's shared memory (pn_onchip.cu): lattices of at most 7168 padded floats per array
 bool pn_onchip_supported(const pn_geom& g);
+// Per-DEVICE opt-in to large dynamic shared memory for the kernels that need it (cudaFuncSetAttribute is per device,
+// not per process): called by pn_create with the handle's device current.
+cudaError_t pn_fused_init_device();
+cudaError_t pn_onchip_init_device();
 cudaError_t pn_launch_cg_onchip(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st);
 
 // Which iteration scheme a PN_OPT_KERNEL value selects on this lattice: 1 = reference two-kernel,
-// 2 = two-kernel with the TMA S4 kernel, 3 = single fused TMA kernel
+// 3 = single fused TMA kernel, 5 = whole loop in one CTA's shared memory
 int pn_resolve_variant(const pn_geom& g, int variant);
 
-// TMA-fed S4 kernel (pn_stencil_tma.cu)
-struct pn_tma_plan;
-bool pn_tma_supported();
-bool pn_tma_plan_build(pn_tma_plan** out, const pn_geom& g, const pn_ptrs& P);
-void pn_tma_plan_free(pn_tma_plan* pl);
-cudaError_t pn_launch_stencil_tma(const pn_tma_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
+bool pn_tma_supported();   // the driver exports cuTensorMapEncodeTiled (pn_fused_tma.cu)

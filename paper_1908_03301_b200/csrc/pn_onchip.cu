@@ -122,15 +122,13 @@ bool pn_onchip_supported(const pn_geom& g) {
     return !(g.wrap[0] | g.wrap[1] | g.wrap[2]) && g.npad + 2 * g.plane <= PN_ONCHIP_MAX_FLOATS;
 }
 
+cudaError_t pn_onchip_init_device() {
+    return cudaFuncSetAttribute(k_cg_onchip, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                7 * PN_ONCHIP_MAX_FLOATS * (int)sizeof(float));
+}
+
 cudaError_t pn_launch_cg_onchip(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st) {
-    static bool attr_done = false;
     const size_t smem = (size_t)7 * (size_t)(g.npad + 2 * g.plane) * sizeof(float);
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_cg_onchip, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             7 * PN_ONCHIP_MAX_FLOATS * (int)sizeof(float));
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
     k_cg_onchip<<<1, TPB, smem, st>>>(g, P, max_launch_iters);
     return cudaGetLastError();
 }

@@ -12,9 +12,9 @@ namespace {
 
 constexpr int TPB = 256;
 
-int grid_for(long long work_items) {
+int grid_for(long long work_items, int sms) {
     long long nb = (work_items + TPB - 1) / TPB;
-    long long cap = (long long)pn_sm_count() * 8;
+    long long cap = (long long)sms * 8;
     if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
     if (nb > cap) nb = cap;
     if (nb < 1) nb = 1;
@@ -189,12 +189,12 @@ __global__ void k_export_cls(pn_geom g, const signed char* __restrict__ cls, sig
 }  // namespace
 
 cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches) {
-    k_residual64<<<grid_for(g.npad), TPB, 0, st>>>(g, P, fused);
+    k_residual64<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P, fused);
     ++*launches;
     return cudaGetLastError();
 }
 cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_flush<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    k_flush<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }
@@ -207,23 +207,23 @@ cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double
 }
 cudaError_t pn_launch_flux(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
     const long long m = g.n / g.n_a;
-    k_flux<<<grid_for(m), TPB, 0, st>>>(g, P);
+    k_flux<<<grid_for(m, g.sms), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }
 cudaError_t pn_launch_export_x(const pn_geom& g, const pn_ptrs& P, double* out, cudaStream_t st, int* launches) {
-    k_export_x<<<grid_for(g.n), TPB, 0, st>>>(g, P.x64, out);
+    k_export_x<<<grid_for(g.n, g.sms), TPB, 0, st>>>(g, P.x64, out);
     ++*launches;
     return cudaGetLastError();
 }
 cudaError_t pn_launch_export_cls(const pn_geom& g, const pn_ptrs& P, signed char* out, int, cudaStream_t st,
                                  int* launches) {
-    k_export_cls<<<grid_for(g.n), TPB, 0, st>>>(g, P.cls, out);
+    k_export_cls<<<grid_for(g.n, g.sms), TPB, 0, st>>>(g, P.cls, out);
     ++*launches;
     return cudaGetLastError();
 }
 cudaError_t pn_launch_dissipation(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_dissipation<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    k_dissipation<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }

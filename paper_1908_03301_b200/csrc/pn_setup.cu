@@ -15,9 +15,9 @@ constexpr int TPB = 256;
 
 __host__ __device__ inline long long cdiv(long long a, long long b) { return (a + b - 1) / b; }
 
-int grid_for(long long work_items) {
+int grid_for(long long work_items, int sms) {
     long long nb = cdiv(work_items, TPB);
-    long long cap = (long long)pn_sm_count() * 8;
+    long long cap = (long long)sms * 8;
     if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
     if (nb > cap) nb = cap;
     if (nb < 1) nb = 1;
@@ -421,18 +421,18 @@ __global__ void k_weights(pn_geom g, pn_ptrs P) {
 }  // namespace
 
 cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_validate<<<grid_for(g.n), TPB, 0, st>>>(g, P.raw[0], P.raw[1], P.raw[2], P.st);
+    k_validate<<<grid_for(g.n, g.sms), TPB, 0, st>>>(g, P.raw[0], P.raw[1], P.raw[2], P.st);
     ++*launches;
     return cudaGetLastError();
 }
 
 cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, bool do_peel, int x0_linear,
                             cudaStream_t st, int* launches) {
-    const int nb = grid_for(g.npad);
+    const int nb = grid_for(g.npad, g.sms);
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];
     long long nface = 1;
     for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
-    const int nbf = grid_for(nface);
+    const int nbf = grid_for(nface, g.sms);
     k_solve_copy<<<nb, TPB, 0, st>>>(g, P);
     ++*launches;
     if (do_label) {
@@ -457,27 +457,27 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, b
 
 // Diagonal scale, ||b||^2 and the scaled weights of the inner system, from the final solve copy.
 cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    const int nb = grid_for(g.npad);
+    const int nb = grid_for(g.npad, g.sms);
     k_scale<<<nb, TPB, 0, st>>>(g, P);
     k_weights<<<nb, TPB, 0, st>>>(g, P);
     *launches += 2;
     if (g.wrap[0] || g.wrap[1] || g.wrap[2]) {
         long long nface = 1;
         for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
-        k_wrap_weights<<<grid_for(nface), TPB, 0, st>>>(g, P);
+        k_wrap_weights<<<grid_for(nface, g.sms), TPB, 0, st>>>(g, P);
         ++*launches;
     }
     return cudaGetLastError();
 }
 
 cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_backfill<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    k_backfill<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }
 
 cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_unpeel<<<grid_for(g.npad), TPB, 0, st>>>(g, P);
+    k_unpeel<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }
@@ -487,7 +487,7 @@ cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st
 cudaError_t pn_launch_wrap_copy(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
     long long nface = 1;
     for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
-    k_wrap_copy<<<grid_for(nface), TPB, 0, st>>>(g, P);
+    k_wrap_copy<<<grid_for(nface, g.sms), TPB, 0, st>>>(g, P);
     ++*launches;
     return cudaGetLastError();
 }

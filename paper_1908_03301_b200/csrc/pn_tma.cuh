@@ -1,5 +1,5 @@
 // pn_tma.cuh -- sm_100a TMA / mbarrier PTX wrappers and the tensor-map encoder shared by the TMA-fed
-// kernels of libpn (pn_stencil_tma.cu, pn_fused_tma.cu).  Not part of the C ABI.
+// kernels of libpn (pn_fused_tma.cu).  Not part of the C ABI.
 #pragma once
 #include <cuda.h>  // CUtensorMap and enums only: the encoder is fetched with cudaGetDriverEntryPoint
 #include <cuda_runtime.h>
@@ -71,13 +71,10 @@ __device__ __forceinline__ void tma_load_3d_hint(float* dst, const CUtensorMap* 
 __device__ __forceinline__ void bar_consumers(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
 
 __device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-// Explicit ld.shared / st.shared.  The tile pointers of the TMA kernels come from a rounded-up dynamic shared-memory
-// base and runtime ring slots, so the compiler cannot prove their address space and emits GENERIC accesses (LD.E / ST.E
-// in SASS) for plain dereferences such as lds4() above.  Measured on one B200, same box (profiles/
-// r01_q_recompute_experiment.md): the explicit form makes k_cg_fused2_tma 11.7 % faster (1.094 -> 0.966 ms per
-// iteration at 512^3) but k_cg_fused_tma 1.6 % SLOWER (0.8997 -> 0.9144 ms; `volatile` pins the order of its loads).
-// pn_fused2_tma.cu has since dropped the integer round trip on its base pointer, so the compiler emits LDS itself
-// (another 2.2 %); these helpers are kept for kernels whose pointers cannot be kept in the shared space.  `volatile`: never merged or moved across the mbarrier waits and barriers.
+// Explicit ld.shared / st.shared for tile pointers whose address space the compiler cannot prove (a rounded-up dynamic
+// shared-memory base makes plain dereferences GENERIC accesses, LD.E / ST.E in SASS).  Which form is faster was measured
+// per kernel (profiles/r01_barrier_placement.md, profiles/r01_q_recompute_experiment.md).  `volatile`: never merged or
+// moved across the mbarrier waits and barriers.
 __device__ __forceinline__ float4 slds4(const float* p) {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(smem_u32(p)));

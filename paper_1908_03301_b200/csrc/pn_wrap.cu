@@ -85,7 +85,7 @@ cudaError_t pn_launch_wrap_fix(const pn_geom& g, const pn_ptrs& P, int fused, cu
     for (int b = 0; b < 3; ++b)
         if (g.wrap[b] && 2 * pn_face_count(g, b) > items) items = 2 * pn_face_count(g, b);
     long long nb = (items + TPB - 1) / TPB;
-    const long long cap = (long long)pn_sm_count() * 4;
+    const long long cap = (long long)g.sms * 4;
     if (nb > cap) nb = cap;
     if (nb < 1) nb = 1;
     k_wrap_fix<<<(int)nb, TPB, 0, st>>>(g, P, fused);
