@@ -63,7 +63,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 struct layout {
     pn_geom g;
     size_t off_raw[3], off_gs[3], off_w[3], off_gsw[3], off_ww[3], off_s, off_x64, off_r, off_p, off_p2, off_q, off_xh, off_r2, off_q2, off_cls, off_slots,
-        off_state, total;
+        off_state, off_xchg, off_gbar, total;
     size_t halo;                // elements in one halo plane
 };
 
@@ -81,6 +81,7 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     g.dir = 0; g.n_a = nx; g.stride_a = 1;
     g.wrap[0] = g.wrap[1] = g.wrap[2] = 0;
     g.sms = 0;
+    g.coop = 0;
     if (g.npad + 2 * g.plane >= (1ll << 31)) return false;
     L->halo = (size_t)g.plane;
     const size_t vec = (size_t)g.npad + 2 * L->halo;   // elements of a padded array with its two halo planes
@@ -101,8 +102,11 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     L->off_r2 = take(vec * 4);
     L->off_q2 = take(vec * 4);
     L->off_cls = take(vec);
-    L->off_slots = take(4 * PN_MAX_BLOCKS * sizeof(double));
+    L->off_slots = take(8 * PN_MAX_BLOCKS * sizeof(double));
     L->off_state = take(sizeof(pn_state));
+    L->off_gbar = take(256);
+    // exchange rows of the persistent 2D kernel (pn_resident.cu); (size_t)-1: not a lattice it handles
+    L->off_xchg = (g.ny == 1 && g.px <= 2048) ? take((size_t)12 * PN_RESIDENT_MAX_CTAS * g.px * 4) : (size_t)-1;
     L->total = o;
     return true;
 }
@@ -166,6 +170,9 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms < 1) sms = 148;
     ctx->g.sms = sms;
+    int coop = 0;
+    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) != cudaSuccess) coop = 0;
+    ctx->g.coop = coop;
     const size_t h = L.halo;
     pn_ptrs& P = ctx->P;
     for (int b = 0; b < 3; ++b) {
@@ -189,11 +196,14 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     P.flags = (int*)P.xh;
     P.slots = (double*)(ctx->ws + L.off_slots);
     P.st = (pn_state*)(ctx->ws + L.off_state);
+    P.gbar = (unsigned int*)(ctx->ws + L.off_gbar);
+    P.xchg = L.off_xchg == (size_t)-1 ? nullptr : (float*)(ctx->ws + L.off_xchg);
     P.scratch = (void*)(ctx->ws + L.off_p);   // p and p2 are adjacent: 8 bytes per padded node
     cudaError_t e = cudaMemsetAsync(ctx->ws, 0, L.total, ctx->stream);
     // large dynamic shared memory is opted into per DEVICE (the attribute is not per process)
     if (e == cudaSuccess && pn_tma_supported()) e = pn_fused_init_device();
     if (e == cudaSuccess) e = pn_onchip_init_device();
+    if (e == cudaSuccess && pn_tma_supported()) e = pn_resident_init_device();
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_state, sizeof(pn_state));
     for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&ctx->ev[i]);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
@@ -230,7 +240,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_X0: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
         case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
-        case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
+        case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0 && value != 6.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
@@ -374,8 +384,9 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + sizeof(P.st->count) + sizeof(P.st->n_peeled), s));
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
-    const int scheme = pn_resolve_variant(g, ctx->variant);
-    const int fused = scheme == 3;   // one kernel per iteration; r double-buffered by iteration parity
+    const int scheme = pn_resolve_variant(g, P, ctx->variant);
+    const int fused = scheme == 3 || scheme == 6;   // one kernel per iteration (deferred residual update, predicted beta)
+    const int bufmode = scheme == 3 ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -406,12 +417,12 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
     CK(cudaMemsetAsync(P.q, 0, vbytes, s));
-    if (fused) CK(cudaMemsetAsync(P.q2, 0, vbytes, s));
+    if (scheme == 3) CK(cudaMemsetAsync(P.q2, 0, vbytes, s));
     // p / p2 double as export staging (pn_get_pressures), halo planes included: clear them whole
     const size_t vhalo = ((size_t)g.npad + 2 * (size_t)g.plane) * 4;
     CK(cudaMemsetAsync(P.p - g.plane, 0, vhalo, s));
     CK(cudaMemsetAsync(P.p2 - g.plane, 0, vhalo, s));
-    CK(pn_launch_residual64(g, P, fused, s, &nl));
+    CK(pn_launch_residual64(g, P, bufmode, s, &nl));
     CK(cudaEventRecord(ctx->ev[1], s));
     rc = read_state(ctx);
     if (rc) return rc;
@@ -457,8 +468,8 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         // Graph path: whole chunks replayed from one executable graph.  With PN_OPT_PROFILE it is used for the single-kernel
         // scheme only (one kernel per iteration: the chunk's device time / iterations run is that kernel's average launch
         // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
-        const bool graph = ctx->use_graph && ctx->chunk > 1 && scheme != 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme);
-        const int per_iter = (fused ? 1 : 2) + (any_wrap ? 1 : 0);
+        const bool graph = ctx->use_graph && ctx->chunk > 1 && scheme < 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme);
+        const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);
         while (true) {
             if (graph) {
                 if (ctx->profile) CK(cudaEventRecord(ctx->pev[0], s));
@@ -475,7 +486,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
                 if (ran > 0) { t_stencil += ta; n_timed += ran; }
-            } else if (ctx->profile && scheme == 5) {   // one launch ran `ran` iterations on chip
+            } else if (ctx->profile && scheme >= 5) {   // one launch ran `ran` iterations (on chip / persistent)
                 const int ran = h->iters - iters_seen;
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
@@ -498,8 +509,8 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
             // iteration has already stepped past it (rr_old), the fused kernel holds it as its measured rr
             const double rr_before = fused ? h->rr : h->rr_old;
             const int flag = h->flag;
-            CK(pn_launch_flush(g, P, s, &nl));
-            CK(pn_launch_residual64(g, P, fused, s, &nl));
+            CK(pn_launch_flush(g, P, bufmode, s, &nl));
+            CK(pn_launch_residual64(g, P, bufmode, s, &nl));
             rc = read_state(ctx);
             if (rc) return rc;
             ++outer;

@@ -149,9 +149,12 @@ int grid_for(long long work_items, int sms) {
 // pair from 64^2 up, profiles/r01_small_lattices.md); 1 = reference two-kernel iteration (independently written
 // cross-check).  The two superseded schemes of round 1 (2: TMA S4 kernel + S5 kernel, 4: q recomputed) are gone;
 // their write-ups remain in profiles/r01_tma_kernel.md and profiles/r01_q_recompute_experiment.md.
-int pn_resolve_variant(const pn_geom& g, int variant) {
-    if (variant == 0) return pn_onchip_supported(g) ? 5 : (pn_tma_supported() ? 3 : 1);
-    if (variant == 5 && !pn_onchip_supported(g)) return pn_tma_supported() ? 3 : 1;   // too large for one SM, or periodic faces
+// 6 = persistent in-place kernel for 2D lattices up to 2048 wide (pn_resident.cu), the automatic choice where it applies.
+int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant) {
+    const int big = pn_tma_supported() ? 3 : 1;
+    if (variant == 0) return pn_onchip_supported(g) ? 5 : (pn_resident_supported(g, P) ? 6 : big);
+    if (variant == 5 && !pn_onchip_supported(g)) return big;   // too large for one SM, or periodic faces
+    if (variant == 6 && !pn_resident_supported(g, P)) return big;   // 3D, wider than 2048, or periodic faces
     return variant;
 }
 
@@ -163,9 +166,9 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     const int nb = grid_for(nvec, g.sms);
     pn_fused_plan* fplan = nullptr;
     if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
-    if (scheme == 5) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu); `iterations` is not a bound here
+    if (scheme == 5 || scheme == 6) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu, pn_resident.cu); `iterations` is not a bound here
         if (ev) cudaEventRecord(ev[0], st);
-        cudaError_t e5 = pn_launch_cg_onchip(g, P, 1 << 30, st);
+        cudaError_t e5 = scheme == 5 ? pn_launch_cg_onchip(g, P, 1 << 30, st) : pn_launch_cg_resident(g, P, 1 << 30, st);
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         *launches += 1;
         return e5;
@@ -182,6 +185,6 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
         if (ev) cudaEventRecord(ev[2 * it + 2], st);
     }
     pn_fused_plan_free(fplan);
-    *launches += ((scheme >= 3 ? 1 : 2) + (wrap ? 1 : 0)) * iterations;
+    *launches += ((scheme == 3 ? 1 : 2) + (wrap ? 1 : 0)) * iterations;
     return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -17,6 +17,7 @@
 #include "../../include/pn.h"
 
 #define PN_MAX_BLOCKS 2048      // upper bound on gridDim.x of every reducing kernel (partial slots)
+#define PN_RESIDENT_MAX_CTAS 160 // upper bound on the cooperative grid of k_cg_resident2d (sizes its exchange array)
 #define PN_CLASS_PAD 7          // internal: pad column (never exported)
 #define PN_CLASS_PEELED 8       // internal: 8 + c = solved node peeled off as a dangling end, hanging from its
                                 // neighbour in direction c (0:+x 1:-x 2:+y 3:-y 4:+z 5:-z); exported as SOLVED
@@ -32,6 +33,7 @@ struct pn_geom {
     long long stride_a;         // element stride along dir (1, px, plane)
     int wrap[3];                // INTERNAL axis wraps around (periodic lateral faces); never `dir`, never a length-1 axis
     int sms;                    // SM count of the handle's device (sizes the persistent grids); set by pn_create
+    int coop;                   // the device launches cooperative kernels (pn_resident.cu)
 };
 
 // ---- periodic lateral faces: the wrap bonds live in small FACE arrays, not in the lattice-shaped ones ----
@@ -195,7 +197,10 @@ struct pn_ptrs {
     signed char* cls;           // node classes
     int* parent;                // union-find forest (aliases q)
     int* flags;                 // per-root inlet/outlet contact bits (aliases xh); after S1d: live bond degree (peeling)
-    double* slots;              // 4 x PN_MAX_BLOCKS partial sums
+    double* slots;              // 8 x PN_MAX_BLOCKS partial sums (4 sums; double-buffered by the persistent kernel)
+    float* xchg;                // 2D lattices up to 2048 wide: boundary rows of r, q, p exchanged between the CTAs of
+                                // k_cg_resident2d, [2 parities][3 vectors][2 * PN_RESIDENT_MAX_CTAS rows][px]; else nullptr
+    unsigned int* gbar;         // arrival counter of its grid barrier
     pn_state* st;
     void* scratch;              // export staging (aliases p, p2)
 };
@@ -206,8 +211,10 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, b
 cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
-cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches);
-cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+// `bufmode`: which buffers hold the vectors of the inner iteration -- 0: two-kernel schemes (r single, p double-buffered
+// by iteration parity), 1: k_cg_fused_tma (r, q, p double-buffered by parity), 2: in place (k_cg_resident2d: P.r, P.q, P.p)
+cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int bufmode, cudaStream_t st, int* launches);
+cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, int bufmode, cudaStream_t st, int* launches);
 cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,
                                 double delta2, int max_iters, int reset_iters, double xskip_min, cudaStream_t st,
                                 int* launches);
@@ -237,8 +244,13 @@ cudaError_t pn_fused_init_device();
 cudaError_t pn_onchip_init_device();
 cudaError_t pn_launch_cg_onchip(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st);
 
+// Persistent in-place iteration for 2D lattices (pn_resident.cu): all iterations up to the next trigger in ONE cooperative launch
+bool pn_resident_supported(const pn_geom& g, const pn_ptrs& P);
+cudaError_t pn_resident_init_device();
+cudaError_t pn_launch_cg_resident(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st);
+
 // Which iteration scheme a PN_OPT_KERNEL value selects on this lattice: 1 = reference two-kernel,
-// 3 = single fused TMA kernel, 5 = whole loop in one CTA's shared memory
-int pn_resolve_variant(const pn_geom& g, int variant);
+// 3 = single fused TMA kernel, 5 = whole loop in one CTA's shared memory, 6 = persistent in-place 2D kernel
+int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant);
 
 bool pn_tma_supported();   // the driver exports cuTensorMapEncodeTiled (pn_fused_tma.cu)

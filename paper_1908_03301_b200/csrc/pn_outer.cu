@@ -25,12 +25,12 @@ int grid_for(long long work_items, int sms) {
 // x64 carries the Dirichlet and pin values on the nodes that are not unknowns, so
 // (b - A x)_i = sum_j g_ij (x_j - x_i) over all six neighbours.  acc[0] = ||r||^2, acc[1] = ||r_hat||^2
 // (of the rounded fp32 values, i.e. exactly what the inner recurrence starts from).
-// `fused`: the single-kernel iteration double-buffers r; the next kernel reads buffer (iters & 1).
-__global__ void k_residual64(pn_geom g, pn_ptrs P, int fused) {
+// `bufmode` 1: the single-kernel iteration double-buffers r; the next kernel reads buffer (iters & 1).
+__global__ void k_residual64(pn_geom g, pn_ptrs P, int bufmode) {
     __shared__ double sm[32];
     __shared__ double tot[2];
     double a0 = 0.0, a1 = 0.0;
-    float* __restrict__ rdst = (fused && (P.st->iters & 1)) ? P.r2 : P.r;
+    float* __restrict__ rdst = (bufmode == 1 && (P.st->iters & 1)) ? P.r2 : P.r;
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const float s = P.s[n];
@@ -72,10 +72,11 @@ __global__ void k_residual64(pn_geom g, pn_ptrs P, int fused) {
 // ---- S7: x64 += s * (x_hat + alpha_x p)  (the pending deferred update included); x_hat = 0 ------
 // Single-kernel scheme with a skipped x_hat update pending (state.xpend): the direction before the last one is
 // recovered as p_{T-1} = (p_T - r_T) / beta_T from the last kernel's p and r, exactly as the next kernel would have.
-__global__ void k_flush(pn_geom g, pn_ptrs P) {
+__global__ void k_flush(pn_geom g, pn_ptrs P, int bufmode) {
     const double ax = P.st->alpha_x;
-    const float* __restrict__ p = (P.st->iters & 1) ? P.p2 : P.p;   // the direction of the last iteration
-    const float* __restrict__ r = (P.st->iters & 1) ? P.r2 : P.r;   // single-kernel scheme: the residual it was built from
+    const bool odd = bufmode != 2 && (P.st->iters & 1);     // in-place scheme: one buffer each
+    const float* __restrict__ p = odd ? P.p2 : P.p;   // the direction of the last iteration
+    const float* __restrict__ r = odd ? P.r2 : P.r;   // single-kernel schemes: the residual it was built from
     const bool pend = P.st->xpend != 0;
     const double c2 = pend ? P.st->alpha2 / P.st->beta_prev : 0.0;
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
@@ -188,13 +189,13 @@ __global__ void k_export_cls(pn_geom g, const signed char* __restrict__ cls, sig
 
 }  // namespace
 
-cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st, int* launches) {
-    k_residual64<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P, fused);
+cudaError_t pn_launch_residual64(const pn_geom& g, const pn_ptrs& P, int bufmode, cudaStream_t st, int* launches) {
+    k_residual64<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P, bufmode);
     ++*launches;
     return cudaGetLastError();
 }
-cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
-    k_flush<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P);
+cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, int bufmode, cudaStream_t st, int* launches) {
+    k_flush<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P, bufmode);
     ++*launches;
     return cudaGetLastError();
 }

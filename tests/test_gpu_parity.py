@@ -125,7 +125,7 @@ def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
 @pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (3, 64), (257, 31)])
 @pytest.mark.parametrize("direction", [0, 1])
 @pytest.mark.parametrize("p", [1.0, 0.7])
-@pytest.mark.parametrize("kernel", [1, 3])
+@pytest.mark.parametrize("kernel", [1, 3, 6])
 def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(shape[0], shape[1], 1, seed=11 + direction, p=p)
@@ -142,7 +142,7 @@ def test_tma_kernel_multi_tile(pn, oracle, shape, direction, kernel):
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("kernel", [3])
+@pytest.mark.parametrize("kernel", [3, 6])
 def test_tma_kernel_2d_wide(pn, oracle, kernel):
     """2D lattice wider than the 2048-node tile of the 2D configuration (x halo between tiles)."""
     from paper_1908_03301_b200 import inputs
@@ -742,3 +742,38 @@ def test_removed_kernel_schemes_are_refused(pn):
             h.set_option(pn.PN_OPT_KERNEL, k)
         assert e.value.code == pn.PN_ERR_ARG
     h.close()
+
+
+# ---- persistent in-place kernel for 2D lattices (pn_resident.cu, scheme 6) ----
+@pytest.mark.parametrize("shape,direction,p", [
+    ((1024, 300), 0, 1.0), ((2048, 160), 1, 1.0), ((600, 1000), 0, 0.7), ((513, 149), 1, 0.8), ((260, 400), 0, 1.0),
+    ((100, 2), 0, 1.0), ((7, 500), 1, 1.0)])
+def test_resident_scheme(pn, oracle, shape, direction, p):
+    """All four row widths (1, 2, 4, 8 TMA boxes), more rows than CTAs and fewer, one row per CTA, ragged widths; the
+    automatic choice for every 2D lattice up to 2048 wide that does not fit one SM.  Iteration counts stay those of the
+    one-launch-per-iteration kernel (same arithmetic per node; only the summation order of the dot products differs)."""
+    from paper_1908_03301_b200 import inputs
+    net = inputs.iid_diluted(shape[0], shape[1], 1, seed=21, p=p)
+    auto, *_ = compare(pn, oracle, net, direction)
+    assert auto.kernel_scheme == (5 if shape[0] * shape[1] < 6000 else 6)
+    k6, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 6})
+    k3, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 3})
+    assert k6.kernel_scheme == 6 and k3.kernel_scheme == 3
+    assert abs(k6.inner_iters - k3.inner_iters) <= 0.05 * k3.inner_iters + 5
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 6, pn.PN_OPT_XDEFER: 0, pn.PN_OPT_DELTA: 0.01})
+
+
+def test_resident_scheme_fallbacks_and_budget(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    wide, *_ = compare(pn, oracle, inputs.iid_diluted(2100, 40, 1, seed=9, p=1.0), 1, opts={pn.PN_OPT_KERNEL: 6})
+    assert wide.kernel_scheme == 3                       # wider than 2048: the tiled kernel
+    cube, *_ = compare(pn, oracle, inputs.cfg4_fbm_cut_3d(40, 36, 33), 0, opts={pn.PN_OPT_KERNEL: 6})
+    assert cube.kernel_scheme == 3                       # 3D
+    per, *_ = compare(pn, oracle, inputs.cfg2_fbm_2d(300, 200), 0, opts={pn.PN_OPT_KERNEL: 6}, periodic=True)
+    assert per.kernel_scheme == 3                        # periodic faces
+    net = inputs.cfg2_fbm_2d(300, 200)
+    info, *_ = gpu_solve(pn, net, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40, pn.PN_OPT_KERNEL: 6})
+    assert info.status == pn.PN_MAX_ITERS and info.kernel_scheme == 6 and info.inner_iters == 40
+    a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: 6})
+    b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: 6})
+    assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]   # bit-reproducible
