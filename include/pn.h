@@ -62,7 +62,7 @@ typedef struct {
     int status;            /* the code pn_solve returned                                            */
     int outer_cycles;      /* fp64 true-residual evaluations  r = b - A x  (S8(a) S3)                */
     int inner_iters;       /* fp32 CG iterations (S8(a) S4+S5), summed over the solve               */
-    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3 or 5) */
+    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3, 5 or 6) */
     double rel_residual;   /* true fp64 ||b - A x||_2 / ||b||_2 over the solved nodes at exit       */
     double b_norm;         /* ||b||_2 of the zero-initial-guess system (S8(c) reading 5)            */
     long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
@@ -76,6 +76,8 @@ typedef struct {
                               they move 8 bytes per node less than the others                        */
     long long n_peeled;    /* solved nodes taken out of the system as dangling ends (PN_OPT_PEEL) and
                               back-filled after the solve; they are counted in n_solved too           */
+    int labels_reused;     /* 1: S1's labelling and peeling were skipped, the classes of the previous solve
+                              still hold (pn_update_conductances / pn_replace_conductances, no bond crossed zero) */
 } pn_info;
 
 /* options for pn_set_option */
@@ -92,11 +94,15 @@ enum {
     PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
-                               memory -- at most 7168 padded floats per array, no periodic faces -- else 3),
+                               memory -- at most 7168 padded floats per array, no periodic faces --, 6 where it
+                               applies, else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept as an independently written cross-check),
                                3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
-                               5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory.
+                               5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory,
+                               6 = 2D lattices whose rows / SMs slabs fit the SMs' shared memory (about 1.2 M nodes,
+                               at most 2048 wide, no periodic faces): ONE persistent cooperative launch per residual
+                               replacement, every CTA keeping its slab on chip, grid barrier per iteration; else 3.
                                (2 and 4 were round-1 experiments, since removed: PN_ERR_ARG)                   */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */
@@ -115,6 +121,10 @@ enum {
                                not wrap                                                             */
     PN_OPT_GRAPH = 9,       /* 1 (default): a chunk of inner iterations is replayed from a CUDA graph (captured
                                once per geometry / direction / scheme); 0: every kernel launched directly  */
+    PN_OPT_REUSE_LABELS = 11, /* 1 (default): a solve that follows pn_update_conductances / pn_replace_conductances (or simply
+                               repeats the previous one) keeps the node classes, pins and peeled set of the previous solve
+                               when no bond went from closed to open or back and direction, PN_OPT_LATERAL, PN_OPT_PEEL
+                               and PN_OPT_SKIP_LABEL are unchanged; 0: S1 is always redone                    */
     PN_OPT_XDEFER = 10      /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
                                iteration, two search directions at once (the earlier one recovered from p and r):
                                40 instead of 44 bytes per node-iteration on average; 0: every iteration    */
@@ -137,6 +147,24 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
  * PN_ERR_VALUE and the handle keeps no network.  Invalidates earlier pressures. */
 int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const float* gz,
                         int pointers_are_device);
+
+/* S8(f) item 4 -- conductances that change between solves ("simulating a flow or transport process that may
+ * take thousands of time steps").  Both calls change the network the handle holds WITHOUT the full S0 + S1 of a new
+ * network: the next pn_solve in the same direction skips the labelling and peeling when no bond went from closed
+ * (g == 0) to open or back (pn_info.labels_reused), rebuilds the solve copy, scaling and weights on the device, and
+ * starts from the pressures of the previous solve (warm start) unless PN_OPT_X0 is 0.  Pressures and fluxes of the
+ * previous solve become unavailable.  Values must be finite and >= 0: PN_ERR_VALUE; a bad axis / node index:
+ * PN_ERR_ARG; on either error the handle keeps no network (as after a failed pn_set_conductances).  Needs a network:
+ * PN_ERR_STATE before pn_set_conductances.
+ *
+ * pn_update_conductances: sparse.  Bond i of the list is the forward bond along `axis[i]` (0 = x, 1 = y, 2 = z; 2D:
+ * 0 or 1) of node `node[i]` (n = i + nx*(j + ny*k)) and takes `value[i]`; `count` entries, all DISTINCT bonds.
+ * Entries whose forward neighbour is off-lattice are stored and ignored as in pn_set_conductances.  HOST or DEVICE
+ * pointers (all three alike).
+ * pn_replace_conductances: all bonds; arguments as pn_set_conductances. */
+int pn_update_conductances(pn_ctx* ctx, long long count, const int* axis, const long long* node, const float* value,
+                           int pointers_are_device);
+int pn_replace_conductances(pn_ctx* ctx, const float* gx, const float* gy, const float* gz, int pointers_are_device);
 
 /* S1..S7: classify and prune clusters for `direction` (0 = x, 1 = y, 2 = z; the axis needs >= 3
  * node planes), then iterate until the true fp64 residual ||b - A x||_2 <= tol * ||b||_2

@@ -37,6 +37,10 @@ struct pn_ctx {
     // options
     int max_iters, chunk, x0_linear, skip_label, variant, profile, peel, lateral;
     int base_closed;            // some in-lattice (non-wrap) bond is closed: from S0's validation
+    // node classes kept from the last solve (S8(f) item 4): reused while no bond crosses zero and nothing they depend on changes
+    int reuse_labels;           // option
+    bool labels_valid, topo_dirty, warm_next;
+    int label_dir, label_lateral, label_peel, label_skip;
     // CUDA graph of one chunk of inner iterations (captured on a private stream, launched on the caller's)
     int use_graph, xdefer;
     cudaStream_t cap_stream;
@@ -163,7 +167,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1;
     ctx->delta = 0.3;   // measured: 0.3 needs 11 % fewer iterations than 0.1 on CFG2 2048^2 and the same on CFG3/4/5
     ctx->last_dir_user = -1;
     // per-handle device facts (no process-global state: handles on different devices are independent)
@@ -245,6 +249,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
+        case PN_OPT_REUSE_LABELS: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->reuse_labels = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
     }
@@ -284,6 +289,9 @@ int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const flo
     ctx->have_g = false;
     ctx->have_solution = false;
     ctx->flux_valid = false;
+    ctx->labels_valid = false;   // a new network: classes, peeling and the warm start are void
+    ctx->topo_dirty = false;
+    ctx->warm_next = false;
     const size_t bytes = (size_t)ctx->g.n * 4;
     const cudaMemcpyKind kind = pointers_are_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     // internal axes: 2D lattices are held as nx x 1 x ny, so user gy feeds the internal z-bond array
@@ -294,7 +302,7 @@ int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const flo
         CK(cudaMemcpyAsync(ctx->raw_store[b], src[b], bytes, kind, ctx->stream));
         ctx->P.raw[b] = ctx->raw_store[b];
     }
-    CK(cudaMemsetAsync(&ctx->P.st->bad_value, 0, 2 * sizeof(int), ctx->stream));
+    CK(cudaMemsetAsync(&ctx->P.st->bad_value, 0, 3 * sizeof(int), ctx->stream));
     int nl = 0;
     CK(pn_launch_validate(ctx->g, ctx->P, ctx->stream, &nl));
     ctx->launches += nl;
@@ -381,7 +389,11 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
 
     // ---- S1 + set-up ----
     CK(cudaEventRecord(ctx->ev[0], s));
-    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + sizeof(P.st->count) + sizeof(P.st->n_peeled), s));
+    // node classes of the previous solve still describe this network? (same direction and options, no bond crossed zero)
+    const bool reuse = ctx->reuse_labels && ctx->labels_valid && !ctx->topo_dirty && ctx->label_dir == g.dir &&
+                       ctx->label_lateral == ctx->lateral && ctx->label_peel == ctx->peel && ctx->label_skip == ctx->skip_label;
+    ctx->labels_valid = false;   // until this solve's S1 has gone through
+    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + (reuse ? 0 : sizeof(P.st->count) + sizeof(P.st->n_peeled)), s));
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     const int scheme = pn_resolve_variant(g, P, ctx->variant);
@@ -390,7 +402,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
-        CK(cudaMemsetAsync(&P.st->bad_value, 0, 2 * sizeof(int), s));
+        CK(cudaMemsetAsync(&P.st->bad_value, 0, 3 * sizeof(int), s));
         CK(pn_launch_wrap_copy(g, P, s, &nl));
         rc = read_state(ctx);
         if (rc) return rc;
@@ -399,9 +411,14 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     }
     const bool do_label = !ctx->skip_label && any_closed;
     const bool do_peel = do_label && ctx->peel;
-    const int x0_mode = (ctx->x0_linear == 2 && !ctx->ever_solved) ? 1 : ctx->x0_linear;   // nothing to warm-start from yet
-    CK(pn_launch_label(g, P, do_label, do_peel, x0_mode, s, &nl));
-    if (do_peel && ctx->peel == 2) {
+    // warm start: asked for (PN_OPT_X0 = 2), or implied by pn_update_conductances / pn_replace_conductances unless the
+    // caller insists on the zero start; nothing to start from before the first solve
+    int x0_mode = ctx->x0_linear;
+    if (ctx->warm_next && x0_mode != 0) x0_mode = 2;
+    if (x0_mode == 2 && !ctx->ever_solved) x0_mode = 1;
+    if (reuse) CK(pn_launch_label_reuse(g, P, x0_mode, s, &nl));
+    else CK(pn_launch_label(g, P, do_label, do_peel, x0_mode, s, &nl));
+    if (!reuse && do_peel && ctx->peel == 2) {
         // automatic: keep the peeling only if it removes at least PN_PEEL_MIN_FRACTION of the unknowns.  Peeled nodes are
         // still streamed (structured storage), so the gain is fewer iterations only; measured on B200:
         // 52 % peeled -> -28 % iterations (CFG3), 3.8 % peeled -> +1.8 % (CFG4: no gain)
@@ -413,6 +430,10 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         }
     }
     CK(pn_launch_scale(g, P, s, &nl));
+    ctx->labels_valid = true;
+    ctx->topo_dirty = false;
+    ctx->warm_next = false;
+    ctx->label_dir = g.dir; ctx->label_lateral = ctx->lateral; ctx->label_peel = ctx->peel; ctx->label_skip = ctx->skip_label;
     // parent / flags aliased q / x_hat: clear the CG vectors before the first iteration
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
@@ -548,6 +569,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         info->n_outlet_only = (long long)h->count[2];
         info->n_floating = (long long)h->count[3];
         info->n_peeled = n_peeled;
+        info->labels_reused = reuse ? 1 : 0;
         if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
         if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
         info->t_stencil_ms = t_stencil;
@@ -555,6 +577,87 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         info->n_timed_iters = n_timed;
     }
     return status;
+}
+
+// Shared tail of the two update calls: read the flags the kernels raised, keep the handle consistent.
+static int finish_update(pn_ctx* ctx, int nl) {
+    ctx->launches += nl;
+    int rc = read_state(ctx);
+    if (rc) return rc;
+    const int bad = ctx->h_state->bad_value;
+    if (bad) {   // some entries may have been written already: the handle keeps no network (as after a failed pn_set_conductances)
+        ctx->have_g = false;
+        ctx->labels_valid = false;
+        return (bad & 1) ? PN_ERR_VALUE : PN_ERR_ARG;
+    }
+    if (ctx->h_state->topo_changed) {
+        // a bond opened or closed: the classes are void, and whether ANY in-lattice bond is closed must be looked at again
+        ctx->topo_dirty = true;
+        CK(cudaMemsetAsync(&ctx->P.st->bad_value, 0, 3 * sizeof(int), ctx->stream));
+        int nl2 = 0;
+        CK(pn_launch_validate(ctx->g, ctx->P, ctx->stream, &nl2));
+        ctx->launches += nl2;
+        rc = read_state(ctx);
+        if (rc) return rc;
+        ctx->base_closed = ctx->h_state->any_closed;
+    }
+    ctx->have_solution = false;
+    ctx->flux_valid = false;
+    ctx->warm_next = true;
+    return PN_OK;
+}
+
+int pn_update_conductances(pn_ctx* ctx, long long count, const int* axis, const long long* node, const float* value,
+                           int pointers_are_device) {
+    if (!ctx || count < 0 || (count > 0 && (!axis || !node || !value))) return PN_ERR_ARG;
+    if (!ctx->have_g) return PN_ERR_STATE;
+    if (count == 0) return PN_OK;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    CK(cudaMemsetAsync(&ctx->P.st->bad_value, 0, 3 * sizeof(int), s));
+    int nl = 0;
+    if (pointers_are_device) {
+        CK(pn_launch_update_raw(ctx->unx, ctx->uny, ctx->unz, ctx->P, ctx->raw_store, count, axis, node, value, ctx->g.sms, s, &nl));
+    } else {
+        // host lists go through the export staging area (8 bytes per padded node), 16 bytes per entry, in pieces
+        const long long cap = (long long)((size_t)ctx->g.npad * 8 / 16);
+        char* stage = (char*)ctx->P.scratch;
+        for (long long o = 0; o < count; o += cap) {
+            const long long m = count - o < cap ? count - o : cap;
+            long long* d_node = (long long*)stage;
+            int* d_axis = (int*)(stage + (size_t)m * 8);
+            float* d_val = (float*)(stage + (size_t)m * 12);
+            CK(cudaMemcpyAsync(d_node, node + o, (size_t)m * 8, cudaMemcpyHostToDevice, s));
+            CK(cudaMemcpyAsync(d_axis, axis + o, (size_t)m * 4, cudaMemcpyHostToDevice, s));
+            CK(cudaMemcpyAsync(d_val, value + o, (size_t)m * 4, cudaMemcpyHostToDevice, s));
+            CK(pn_launch_update_raw(ctx->unx, ctx->uny, ctx->unz, ctx->P, ctx->raw_store, m, d_axis, d_node, d_val, ctx->g.sms, s, &nl));
+        }
+    }
+    return finish_update(ctx, nl);
+}
+
+int pn_replace_conductances(pn_ctx* ctx, const float* gx, const float* gy, const float* gz, int pointers_are_device) {
+    if (!ctx || !gx || !gy) return PN_ERR_ARG;
+    if ((ctx->unz == 1) != (gz == nullptr)) return PN_ERR_ARG;
+    if (!ctx->have_g) return PN_ERR_STATE;
+    device_guard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError(), "cudaSetDevice");
+    cudaStream_t s = ctx->stream;
+    CK(cudaMemsetAsync(&ctx->P.st->bad_value, 0, 3 * sizeof(int), s));
+    const float* src[3] = {gx, ctx->is2d ? nullptr : gy, ctx->is2d ? gy : gz};
+    const size_t bytes = (size_t)ctx->g.n * 4;
+    int nl = 0;
+    for (int b = 0; b < 3; ++b) {
+        if (!src[b]) continue;
+        const float* d_src = src[b];
+        if (!pointers_are_device) {   // through the export staging area (8 bytes per padded node >= one array)
+            CK(cudaMemcpyAsync(ctx->P.scratch, src[b], bytes, cudaMemcpyHostToDevice, s));
+            d_src = (const float*)ctx->P.scratch;
+        }
+        CK(pn_launch_replace_raw(ctx->g, ctx->raw_store[b], d_src, b, ctx->P.st, s, &nl));
+    }
+    return finish_update(ctx, nl);
 }
 
 int pn_solve(pn_ctx* ctx, int direction, double tol, pn_info* info) {

@@ -76,6 +76,7 @@ struct pn_state {
     int max_iters;
     int bad_value;              // set by the validation kernel
     int any_closed;             // some in-lattice bond has g == 0
+    int topo_changed;           // pn_update_conductances / pn_replace_conductances: some bond went from closed to open or back
     unsigned int ticket;        // last-block-done counter (always 0 between kernels)
 };
 
@@ -208,6 +209,16 @@ struct pn_ptrs {
 cudaError_t pn_launch_validate(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, bool do_peel, int x0_linear,
                             cudaStream_t st, int* launches);
+// S1 with the node classes of the previous solve kept (no bond crossed zero since): solve copy + pruning only;
+// x0_mode 0 / 1 re-initialise the solved nodes' pressures, 2 keeps them (warm start)
+cudaError_t pn_launch_label_reuse(const pn_geom& g, const pn_ptrs& P, int x0_mode, cudaStream_t st, int* launches);
+// sparse / full replacement of conductances in the caller-layout copy (pn_update_conductances, pn_replace_conductances):
+// validates, notes closed bonds and zero crossings in the state (bad_value: 1 = value, 2 = index)
+cudaError_t pn_launch_update_raw(int unx, int uny, int unz, const pn_ptrs& P, float* const raw[3], long long count,
+                                 const int* axis, const long long* node, const float* value, int sms, cudaStream_t st,
+                                 int* launches);
+cudaError_t pn_launch_replace_raw(const pn_geom& g, float* raw, const float* src, int axis_internal, pn_state* state,
+                                  cudaStream_t st, int* launches);
 cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);

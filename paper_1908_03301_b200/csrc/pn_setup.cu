@@ -42,6 +42,60 @@ __global__ void k_validate(pn_geom g, const float* __restrict__ r0, const float*
     }
 }
 
+// ---- S8(f) item 4: conductances that change between solves ("thousands of time steps") ----------------------
+// Sparse form: bond (axis[i], node[i]) of the CALLER's lattice (forward-bond convention) takes value[i].  Entries must be
+// distinct.  2D lattices: caller axis 1 is the internal z-bond array (raw[2]).
+__global__ void k_update_raw(int unx, int uny, int unz, float* r0, float* r1, float* r2, long long count,
+                             const int* __restrict__ axis, const long long* __restrict__ node,
+                             const float* __restrict__ value, pn_state* st) {
+    const long long N = (long long)unx * uny * unz;
+    const bool is2d = unz == 1;
+    int bad = 0, closed = 0, topo = 0;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < count; t += (long long)gridDim.x * blockDim.x) {
+        const int a = axis[t];
+        const long long n = node[t];
+        if (a < 0 || a > (is2d ? 1 : 2) || n < 0 || n >= N) { bad |= 2; continue; }
+        const float v = value[t];
+        if (!(v >= 0.0f) || isinf(v)) { bad |= 1; continue; }
+        float* arr = a == 0 ? r0 : (is2d ? r2 : (a == 1 ? r1 : r2));
+        const float old = arr[n];
+        topo |= (old == 0.0f) != (v == 0.0f);
+        closed |= (v == 0.0f);
+        arr[n] = v;
+    }
+    bad = __syncthreads_or(bad & 1) | (__syncthreads_or(bad & 2) ? 2 : 0);
+    closed = __syncthreads_or(closed);
+    topo = __syncthreads_or(topo);
+    if (threadIdx.x == 0) {
+        if (bad) atomicOr(&st->bad_value, bad);
+        if (closed) atomicOr(&st->any_closed, 1);
+        if (topo) atomicOr(&st->topo_changed, 1);
+    }
+}
+
+// Full form, one array at a time: raw <- src with S0's validation of the in-lattice bonds (which entries are bonds
+// depends on the INTERNAL axis b of this array) and the zero-crossing note.
+__global__ void k_replace_raw(pn_geom g, float* __restrict__ raw, const float* __restrict__ src, int b, pn_state* st) {
+    int bad = 0, closed = 0, topo = 0;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.n; n += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(n % g.nx), j = (int)((n / g.nx) % g.ny), k = (int)(n / ((long long)g.nx * g.ny));
+        const float v = src[n], old = raw[n];
+        const bool bond = b == 0 ? i + 1 < g.nx : (b == 1 ? j + 1 < g.ny : k + 1 < g.nz);
+        if (bond) { bad |= !(v >= 0.0f) || isinf(v); closed |= (v == 0.0f); }
+        // entries that are not bonds without periodic faces may become bonds with them: their crossings count too
+        topo |= (old == 0.0f) != (v == 0.0f);
+        raw[n] = v;
+    }
+    bad = __syncthreads_or(bad);
+    closed = __syncthreads_or(closed);
+    topo = __syncthreads_or(topo);
+    if (threadIdx.x == 0) {
+        if (bad) atomicOr(&st->bad_value, 1);
+        if (closed) atomicOr(&st->any_closed, 1);
+        if (topo) atomicOr(&st->topo_changed, 1);
+    }
+}
+
 struct coords { int i, j, k; };
 __device__ __forceinline__ coords coords_of(const pn_geom& g, long long n) {
     coords c;
@@ -267,6 +321,17 @@ __global__ void k_classify(pn_geom g, pn_ptrs P, int x0_linear) {
     if (threadIdx.x < 4 && sc[threadIdx.x]) atomicAdd(&P.st->count[threadIdx.x], sc[threadIdx.x]);
 }
 
+// Label reuse with PN_OPT_X0 = 0 / 1: the solved nodes (peeled ones included) go back to the zero / linear start
+__global__ void k_reset_x0(pn_geom g, pn_ptrs P, int x0_linear) {
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
+        const int c = P.cls[n];
+        if (c == PN_CLASS_SOLVED || c >= PN_CLASS_PEELED) {
+            const coords cc = coords_of(g, n);
+            P.x64[n] = x0_linear ? 1.0 - (double)along(g, cc) / (double)(g.n_a - 1) : 0.0;
+        }
+    }
+}
+
 // ---- S1e: prune -- zero every bond that has a pinned end (pinned rows get a zero diagonal) ------
 __global__ void k_prune(pn_geom g, pn_ptrs P) {
     const long long stride[3] = {1, g.px, g.plane};
@@ -452,6 +517,39 @@ cudaError_t pn_launch_label(const pn_geom& g, const pn_ptrs& P, bool do_label, b
         k_classify<false><<<nb, TPB, 0, st>>>(g, P, x0_linear);
         ++*launches;
     }
+    return cudaGetLastError();
+}
+
+// S1 when no bond crossed zero since the classes were computed (same direction and options): the classes -- and with them
+// the pins, the peeled set and the counts -- stand; only the values of the solve copy change.  A bond survives iff both
+// ends are Dirichlet or solved nodes (k_prune's rule; peeled nodes have class codes above SOLVED, so their one bond goes).
+cudaError_t pn_launch_label_reuse(const pn_geom& g, const pn_ptrs& P, int x0_mode, cudaStream_t st, int* launches) {
+    const int nb = grid_for(g.npad, g.sms);
+    k_solve_copy<<<nb, TPB, 0, st>>>(g, P);
+    k_prune<<<nb, TPB, 0, st>>>(g, P);
+    *launches += 2;
+    if (g.wrap[0] || g.wrap[1] || g.wrap[2]) {
+        long long nface = 1;
+        for (int b = 0; b < 3; ++b) if (g.wrap[b] && pn_face_count(g, b) > nface) nface = pn_face_count(g, b);
+        k_wrap_prune<<<grid_for(nface, g.sms), TPB, 0, st>>>(g, P);
+        ++*launches;
+    }
+    if (x0_mode != 2) { k_reset_x0<<<nb, TPB, 0, st>>>(g, P, x0_mode); ++*launches; }
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_update_raw(int unx, int uny, int unz, const pn_ptrs& P, float* const raw[3], long long count,
+                                 const int* axis, const long long* node, const float* value, int sms, cudaStream_t st,
+                                 int* launches) {
+    k_update_raw<<<grid_for(count, sms), TPB, 0, st>>>(unx, uny, unz, raw[0], raw[1], raw[2], count, axis, node, value, P.st);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_replace_raw(const pn_geom& g, float* raw, const float* src, int axis_internal, pn_state* state,
+                                  cudaStream_t st, int* launches) {
+    k_replace_raw<<<grid_for(g.n, g.sms), TPB, 0, st>>>(g, raw, src, axis_internal, state);
+    ++*launches;
     return cudaGetLastError();
 }
 

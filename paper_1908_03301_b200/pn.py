@@ -24,13 +24,14 @@ LIB_PATH = os.path.join(HERE, "libpn.so")
 PN_OK, PN_NO_SPANNING_CLUSTER, PN_MAX_ITERS = 0, 1, 2
 PN_ERR_ARG, PN_ERR_STATE, PN_ERR_VALUE, PN_ERR_WORKSPACE, PN_ERR_CUDA, PN_ERR_BREAKDOWN = -1, -2, -3, -4, -5, -6
 (PN_OPT_MAX_ITERS, PN_OPT_DELTA, PN_OPT_X0, PN_OPT_CHUNK, PN_OPT_SKIP_LABEL, PN_OPT_KERNEL, PN_OPT_PROFILE,
- PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER) = range(11)
+ PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER, PN_OPT_REUSE_LABELS) = range(12)
 CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CLASS_FLOATING = range(6)
 
 # every symbol include/pn.h declares (tests check that the library exports each of them)
 SYMBOLS = ("pn_workspace_bytes", "pn_create", "pn_set_conductances", "pn_solve", "pn_get_pressures",
            "pn_get_classes", "pn_flux", "pn_set_option", "pn_launch_count", "pn_destroy", "pn_strerror",
-           "pn_last_error", "pn_residual_history", "pn_dissipation")
+           "pn_last_error", "pn_residual_history", "pn_dissipation", "pn_update_conductances",
+           "pn_replace_conductances")
 
 
 class PnInfo(ctypes.Structure):
@@ -41,7 +42,7 @@ class PnInfo(ctypes.Structure):
                 ("t_label_ms", ctypes.c_double), ("t_solve_ms", ctypes.c_double),
                 ("t_stencil_ms", ctypes.c_double), ("t_update_ms", ctypes.c_double),
                 ("n_timed_iters", ctypes.c_int), ("n_xskip", ctypes.c_int),
-                ("n_peeled", ctypes.c_longlong)]
+                ("n_peeled", ctypes.c_longlong), ("labels_reused", ctypes.c_int)]
 
 
 @dataclass
@@ -63,6 +64,7 @@ class SolveInfo:
     kernel_scheme: int = 0
     n_peeled: int = 0
     n_xskip: int = 0
+    labels_reused: int = 0
 
 
 class PnError(RuntimeError):
@@ -92,6 +94,10 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.pn_create.restype = ctypes.c_int
     lib.pn_set_conductances.argtypes = [vp, vp, vp, vp, ctypes.c_int]
     lib.pn_set_conductances.restype = ctypes.c_int
+    lib.pn_update_conductances.argtypes = [vp, ctypes.c_longlong, vp, vp, vp, ctypes.c_int]
+    lib.pn_update_conductances.restype = ctypes.c_int
+    lib.pn_replace_conductances.argtypes = [vp, vp, vp, vp, ctypes.c_int]
+    lib.pn_replace_conductances.restype = ctypes.c_int
     lib.pn_solve.argtypes = [vp, ctypes.c_int, ctypes.c_double, ctypes.POINTER(PnInfo)]
     lib.pn_solve.restype = ctypes.c_int
     lib.pn_get_pressures.argtypes = [vp, vp, ctypes.c_int]
@@ -161,7 +167,7 @@ class Network:
         self._check(self._lib.pn_set_option(self._h, key, float(value)))
 
     # -- S0 --------------------------------------------------------------------------------------
-    def set_conductances(self, gx, gy, gz=None):
+    def set_conductances(self, gx, gy, gz=None, _entry="pn_set_conductances"):
         """gx, gy, gz: numpy float32 arrays / torch tensors of nx*ny*nz entries (shape (nz, ny, nx))."""
         torch = self._torch
         import numpy as np
@@ -191,7 +197,36 @@ class Network:
                 raise PnError(PN_ERR_ARG, "mix of host and device conductance arrays")
             keep.append(t)
             ptrs.append(ctypes.c_void_p(ptr))
-        rc = self._lib.pn_set_conductances(self._h, ptrs[0], ptrs[1], ptrs[2], 1 if on_device else 0)
+        rc = getattr(self._lib, _entry)(self._h, ptrs[0], ptrs[1], ptrs[2], 1 if on_device else 0)
+        del keep
+        self._check(rc)
+
+    def replace_conductances(self, gx, gy, gz=None):
+        """pn_replace_conductances: new values for all bonds of the network the handle holds (labels and warm start kept
+        when no bond crosses zero).  Arguments as set_conductances."""
+        self.set_conductances(gx, gy, gz, _entry="pn_replace_conductances")
+
+    def update_conductances(self, axis, node, value):
+        """pn_update_conductances: sparse update.  axis (int32), node (int64), value (float32): numpy arrays or torch
+        tensors of equal length, all on the host or all on the device."""
+        torch = self._torch
+        import numpy as np
+        want = (("int32", torch.int32), ("int64", torch.int64), ("float32", torch.float32))
+        keep, ptrs, dev = [], [], None
+        for a, (npd, td) in zip((axis, node, value), want):
+            if isinstance(a, torch.Tensor):
+                t = a.detach().to(td).contiguous()
+                d, ptr, n = t.is_cuda, t.data_ptr(), t.numel()
+            else:
+                t = np.ascontiguousarray(a, dtype=npd)
+                d, ptr, n = False, t.ctypes.data, t.size
+            if dev is None:
+                dev, count = d, n
+            elif dev != d or n != count:
+                raise PnError(PN_ERR_ARG, "update lists differ in length or in where they live")
+            keep.append(t)
+            ptrs.append(ctypes.c_void_p(ptr))
+        rc = self._lib.pn_update_conductances(self._h, count, ptrs[0], ptrs[1], ptrs[2], 1 if dev else 0)
         del keep
         self._check(rc)
 
@@ -202,7 +237,8 @@ class Network:
         self._check(rc, ok=tuple(accept))
         return SolveInfo(rc, info.outer_cycles, info.inner_iters, info.rel_residual, info.b_norm, info.n_solved,
                          info.n_inlet_only, info.n_outlet_only, info.n_floating, info.t_label_ms, info.t_solve_ms,
-                         info.t_stencil_ms, info.t_update_ms, info.n_timed_iters, info.kernel_scheme, info.n_peeled, info.n_xskip)
+                         info.t_stencil_ms, info.t_update_ms, info.n_timed_iters, info.kernel_scheme, info.n_peeled, info.n_xskip,
+                         info.labels_reused)
 
     def pressures(self, out=None):
         """fp64 pressures on all nodes as a CUDA tensor of shape (nz, ny, nx)."""
