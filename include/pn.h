@@ -62,7 +62,7 @@ typedef struct {
     int status;            /* the code pn_solve returned                                            */
     int outer_cycles;      /* fp64 true-residual evaluations  r = b - A x  (S8(a) S3)                */
     int inner_iters;       /* fp32 CG iterations (S8(a) S4+S5), summed over the solve               */
-    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3, 5 or 6) */
+    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3, 5 or 6), or 7 = compacted unknowns (PN_OPT_COMPACT) */
     double rel_residual;   /* true fp64 ||b - A x||_2 / ||b||_2 over the solved nodes at exit       */
     double b_norm;         /* ||b||_2 of the zero-initial-guess system (S8(c) reading 5)            */
     long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
@@ -76,6 +76,7 @@ typedef struct {
                               they move 8 bytes per node less than the others                        */
     long long n_peeled;    /* solved nodes taken out of the system as dangling ends (PN_OPT_PEEL) and
                               back-filled after the solve; they are counted in n_solved too           */
+    long long n_unknowns;  /* unknowns of the inner linear system: n_solved - n_peeled                     */
     int labels_reused;     /* 1: S1's labelling and peeling were skipped, the classes of the previous solve
                               still hold (pn_update_conductances / pn_replace_conductances, no bond crossed zero) */
 } pn_info;
@@ -125,6 +126,13 @@ enum {
                                repeats the previous one) keeps the node classes, pins and peeled set of the previous solve
                                when no bond went from closed to open or back and direction, PN_OPT_LATERAL, PN_OPT_PEEL
                                and PN_OPT_SKIP_LABEL are unchanged; 0: S1 is always redone                    */
+    PN_OPT_COMPACT = 12,    /* active-node compaction (S8(f) item 1; the paper's critical slow-down case): the
+                               inner iteration runs on the UNKNOWNS only, stored contiguously with a neighbour
+                               table (kernel_scheme 7; 64 bytes per unknown and iteration instead of 40 per lattice
+                               node).  0: never, 1: whenever it applies, 2 (default): when at most 0.45 of the padded
+                               lattice nodes are unknowns (e.g. configs[2] after peeling: 0.33).  Applies to schemes
+                               3 / 0 on lattices without periodic faces whose table fits the workspace; pressures of
+                               all nodes are unchanged                                                        */
     PN_OPT_XDEFER = 10      /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
                                iteration, two search directions at once (the earlier one recovered from p and r):
                                40 instead of 44 bytes per node-iteration on average; 0: every iteration    */

@@ -39,6 +39,7 @@ struct pn_ctx {
     int base_closed;            // some in-lattice (non-wrap) bond is closed: from S0's validation
     // node classes kept from the last solve (S8(f) item 4): reused while no bond crosses zero and nothing they depend on changes
     int reuse_labels;           // option
+    int compact;                // option: active-node compaction 0 off, 1 on, 2 automatic
     bool labels_valid, topo_dirty, warm_next;
     int label_dir, label_lateral, label_peel, label_skip;
     // CUDA graph of one chunk of inner iterations (captured on a private stream, launched on the caller's)
@@ -47,6 +48,8 @@ struct pn_ctx {
     cudaGraphExec_t graph_exec;
     pn_geom graph_g;
     int graph_scheme, graph_chunk;
+    long long graph_cm, graph_clong;   // compact scheme: the captured kernels carry pointers that depend on these
+    pn_cptrs C;                 // compact arrays of the current solve (scheme 7)
     cudaEvent_t* pev;           // event pool for PN_OPT_PROFILE (2*chunk+1), created on demand
     int pev_n;
     double delta;
@@ -61,6 +64,7 @@ struct pn_ctx {
 namespace {
 
 constexpr double PN_PEEL_MIN_FRACTION = 0.10;
+constexpr double PN_COMPACT_MAX_FRACTION = 0.45;   // automatic compaction: unknowns per padded lattice node at most this
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -167,7 +171,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1; ctx->compact = 2;
     ctx->delta = 0.3;   // measured: 0.3 needs 11 % fewer iterations than 0.1 on CFG2 2048^2 and the same on CFG3/4/5
     ctx->last_dir_user = -1;
     // per-handle device facts (no process-global state: handles on different devices are independent)
@@ -249,6 +253,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
+        case PN_OPT_COMPACT: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->compact = (int)value; return PN_OK;
         case PN_OPT_REUSE_LABELS: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->reuse_labels = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
         default: return PN_ERR_ARG;
@@ -332,8 +337,8 @@ static int read_state(pn_ctx* ctx) {
 // of a solve and every later solve with the same geometry, direction, scheme and chunk length.  Captured on a
 // private stream (the caller's may be the legacy default stream, which cannot be captured); nothing executes
 // there.  Returns false (graph_exec == nullptr) when capture is unavailable: the caller launches directly.
-static bool ensure_graph(pn_ctx* ctx, int scheme) {
-    if (ctx->graph_exec && ctx->graph_scheme == scheme && ctx->graph_chunk == ctx->chunk &&
+static bool ensure_graph(pn_ctx* ctx, int scheme, long long cm, long long clong) {
+    if (ctx->graph_exec && ctx->graph_scheme == scheme && ctx->graph_chunk == ctx->chunk && ctx->graph_cm == cm && ctx->graph_clong == clong &&
         same_geom(ctx->graph_g, ctx->g))
         return true;
     if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
@@ -345,7 +350,7 @@ static bool ensure_graph(pn_ctx* ctx, int scheme) {
     int dummy = 0;
     // warm the launch path once outside capture is not needed: function attributes are set by the launchers themselves
     if (cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return false; }
-    cudaError_t e = pn_launch_inner(ctx->g, ctx->P, ctx->chunk, scheme, ctx->cap_stream, &dummy, nullptr);
+    cudaError_t e = pn_launch_inner(ctx->g, ctx->P, ctx->chunk, scheme, ctx->cap_stream, &dummy, nullptr, &ctx->C);
     cudaGraph_t graph = nullptr;
     cudaError_t e2 = cudaStreamEndCapture(ctx->cap_stream, &graph);
     if (e != cudaSuccess || e2 != cudaSuccess || !graph) {
@@ -359,6 +364,8 @@ static bool ensure_graph(pn_ctx* ctx, int scheme) {
     ctx->graph_g = ctx->g;
     ctx->graph_scheme = scheme;
     ctx->graph_chunk = ctx->chunk;
+    ctx->graph_cm = cm;
+    ctx->graph_clong = clong;
     return true;
 }
 
@@ -396,9 +403,9 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + (reuse ? 0 : sizeof(P.st->count) + sizeof(P.st->n_peeled)), s));
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
-    const int scheme = pn_resolve_variant(g, P, ctx->variant);
-    const int fused = scheme == 3 || scheme == 6;   // one kernel per iteration (deferred residual update, predicted beta)
-    const int bufmode = scheme == 3 ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
+    int scheme = pn_resolve_variant(g, P, ctx->variant);
+    int fused = scheme == 3 || scheme == 6;   // deferred residual update + predicted beta (the state holds the measured r.r)
+    int bufmode = scheme == 3 ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -443,7 +450,26 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     const size_t vhalo = ((size_t)g.npad + 2 * (size_t)g.plane) * 4;
     CK(cudaMemsetAsync(P.p - g.plane, 0, vhalo, s));
     CK(cudaMemsetAsync(P.p2 - g.plane, 0, vhalo, s));
+    // ---- active-node compaction (S8(f) item 1): when few lattice nodes are unknowns, iterate on the unknowns only ----
+    // 64 bytes per unknown and iteration against 40 per lattice node: automatic below 0.45 unknowns per padded node.  The
+    // compact arrays live in lattice-shaped arrays (npad entries each): pn_compact_fits.
+    long long cm = 0, clong = 0;
+    // (automatic only with the automatic kernel choice: an explicit PN_OPT_KERNEL is honoured unless PN_OPT_COMPACT = 1)
+    if ((ctx->compact == 1 || (ctx->compact == 2 && ctx->variant == 0)) && !any_wrap && (scheme == 3 || scheme == 1)) {
+        CK(pn_launch_compact_count(g, P, s, &nl));
+        rc = read_state(ctx);
+        if (rc) return rc;
+        const long long m = (long long)ctx->h_state->cm, nl_rows = (long long)ctx->h_state->clong;
+        const bool want = ctx->compact == 1 || (double)m <= PN_COMPACT_MAX_FRACTION * (double)g.npad;
+        if (want && pn_compact_fits(g, m, nl_rows)) {
+            ctx->C = pn_compact_ptrs(P, m, nl_rows);
+            CK(pn_launch_compact_build(g, P, ctx->C, m, s, &nl));
+            cm = m; clong = nl_rows;
+            scheme = 7; fused = 1; bufmode = 2;
+        }
+    }
     CK(pn_launch_residual64(g, P, bufmode, s, &nl));
+    if (cm) CK(pn_launch_compact_gather(g, P, ctx->C, cm, s, &nl));
     CK(cudaEventRecord(ctx->ev[1], s));
     rc = read_state(ctx);
     if (rc) return rc;
@@ -475,7 +501,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         rn = 0.0;
     } else if (rn > tol * nb) {
         const double delta2 = ctx->delta * ctx->delta;
-        const double xskip_min = (fused && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
+        const double xskip_min = (fused && scheme != 7 && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
         auto target_for = [&](double rn_true, double rr_true) {
             // proxy of the fp64 exit test in the scaled norm: ||r|| / ||r_hat|| measured at this replacement
             const double c = rn_true / sqrt(rr_true);
@@ -489,8 +515,8 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         // Graph path: whole chunks replayed from one executable graph.  With PN_OPT_PROFILE it is used for the single-kernel
         // scheme only (one kernel per iteration: the chunk's device time / iterations run is that kernel's average launch
         // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
-        const bool graph = ctx->use_graph && ctx->chunk > 1 && scheme < 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme);
-        const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);
+        const bool graph = ctx->use_graph && ctx->chunk > 1 && (scheme < 5 || scheme == 7) && !(ctx->profile && !fused) && ensure_graph(ctx, scheme, cm, clong);
+        const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);   // (scheme 7: two kernels, never with wrap)
         while (true) {
             if (graph) {
                 if (ctx->profile) CK(cudaEventRecord(ctx->pev[0], s));
@@ -498,7 +524,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 if (ctx->profile) CK(cudaEventRecord(ctx->pev[1], s));
                 nl += per_iter * ctx->chunk;
             } else {
-                CK(pn_launch_inner(g, P, ctx->chunk, scheme, s, &nl, ctx->profile ? ctx->pev : nullptr));
+                CK(pn_launch_inner(g, P, ctx->chunk, scheme, s, &nl, ctx->profile ? ctx->pev : nullptr, &ctx->C));
             }
             rc = read_state(ctx);
             if (rc) return rc;
@@ -507,7 +533,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
                 if (ran > 0) { t_stencil += ta; n_timed += ran; }
-            } else if (ctx->profile && scheme >= 5) {   // one launch ran `ran` iterations (on chip / persistent)
+            } else if (ctx->profile && (scheme == 5 || scheme == 6)) {   // one launch ran `ran` iterations (on chip / persistent)
                 const int ran = h->iters - iters_seen;
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
@@ -530,8 +556,10 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
             // iteration has already stepped past it (rr_old), the fused kernel holds it as its measured rr
             const double rr_before = fused ? h->rr : h->rr_old;
             const int flag = h->flag;
-            CK(pn_launch_flush(g, P, bufmode, s, &nl));
+            if (cm) CK(pn_launch_compact_flush(g, P, ctx->C, cm, s, &nl));
+            else CK(pn_launch_flush(g, P, bufmode, s, &nl));
             CK(pn_launch_residual64(g, P, bufmode, s, &nl));
+            if (cm) CK(pn_launch_compact_gather(g, P, ctx->C, cm, s, &nl));
             rc = read_state(ctx);
             if (rc) return rc;
             ++outer;
@@ -570,6 +598,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         info->n_floating = (long long)h->count[3];
         info->n_peeled = n_peeled;
         info->labels_reused = reuse ? 1 : 0;
+        info->n_unknowns = cm ? cm : n_solved - n_peeled;
         if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
         if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
         info->t_stencil_ms = t_stencil;

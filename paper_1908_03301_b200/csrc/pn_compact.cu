@@ -1,0 +1,394 @@
+// pn_compact.cu -- active-node compaction (second half): the fp32 inner CG iteration on the
+// UNKNOWNS only, stored contiguously with an ELL-3 + overflow neighbour table, for diluted networks in which most lattice nodes are
+// not unknowns (pinned clusters, Dirichlet planes, peeled dangling ends).
+//
+// Why a gather form and not bricks (profiles/r02_compaction.md): near the threshold (configs[2],
+// p = 0.30) one third of the lattice nodes are unknowns after peeling (the critical slow-down case), but
+// they are spread uniformly: 12.7 % of the 8-node x-segments and 0.1 % of the 32-node ones hold no unknown, so dropping
+// empty segments or tiles of the structured kernel would skip next to nothing.  The 2-core that remains has mean
+// degree 2.37 (69 % of its nodes have two bonds, 25 % three), so the table is ELL of width 3 -- three (index, weight)
+// slots per row, structure of arrays, unused slots pointing at the row itself with weight 0 -- and the 6 % of rows with
+// more bonds keep entries 3..6 in an overflow record their third slot points to: 24 bytes per row + 32 per long row, no
+// row-pointer indirection (a CSR version measured 136 us per iteration on configs[2] against 117 us structured: its
+// rowptr -> col -> p chain of dependent loads was latency-bound).
+//
+// Iteration t (same recurrences as k_cg_fused_tma: deferred residual update, beta predicted from r.r, r.q, q.q, so that
+// both kernels know their scalars at launch; all sums fp32 products -> fp64, fixed-order grid reduction):
+//   k_cupdate:  r_t = r - alpha_{t-1} q ;  x_hat += alpha_{t-1} p ;  p_t = r_t + beta_t p ;  r_t.r_t      (pure stream, 28 B)
+//   k_cspmv:    q_t = p_t - sum_k val_k p_t[col_k] ;  p.q, r.q, q.q  -> alpha_t, beta_{t+1}, flags        (36 B + gathers)
+// = 64 bytes per UNKNOWN and iteration, against 40 bytes per LATTICE NODE for the structured kernel: pays when fewer
+// than ~0.45 of the padded lattice nodes are unknowns.  Unknowns are numbered in lattice order, so x-neighbours are
+// adjacent and y / z neighbours a fixed few thousand entries away: the gathers are served by L1 / L2.
+// The fp64 outer steps stay on the lattice (k_residual64 writes r_hat there); k_cgather / k_cflush move r_hat and the
+// correction between the two numberings.  No periodic faces (those lattices keep the structured kernels).
+#include "pn_internal.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+constexpr int SCAN_T = 1024;                 // threads of the scan kernels
+
+int grid_for(long long work_items, int sms) {
+    long long nb = (work_items + TPB - 1) / TPB;
+    long long cap = (long long)sms * 8;
+    if (cap > PN_MAX_BLOCKS) cap = PN_MAX_BLOCKS;
+    if (nb > cap) nb = cap;
+    if (nb < 1) nb = 1;
+    return (int)nb;
+}
+
+// one scan over (unknown count, long-row count) numbers the unknowns AND the overflow records
+struct scan2 { unsigned long long n, e; };
+__device__ __forceinline__ scan2 operator+(const scan2& a, const scan2& b) { return scan2{a.n + b.n, a.e + b.e}; }
+
+// (is unknown, is a long row) of lattice node n: an unknown has a non-zero Jacobi scale; a table entry per non-zero
+// scaled weight (weights towards Dirichlet, pinned and peeled nodes are zero: they live in the diagonal and in b);
+// long = more than three entries
+__device__ __forceinline__ scan2 node_counts(const pn_geom& g, const pn_ptrs& P, long long n) {
+    scan2 v{0ull, 0ull};
+    if (P.s[n] != 0.f) {
+        v.n = 1ull;
+        const int deg = (P.w[2][n - g.plane] != 0.f) + (P.w[1][n - g.px] != 0.f) + (P.w[0][n - 1] != 0.f) +
+                        (P.w[0][n] != 0.f) + (P.w[1][n] != 0.f) + (P.w[2][n] != 0.f);
+        v.e = deg > 3 ? 1ull : 0ull;
+    }
+    return v;
+}
+
+__device__ __forceinline__ scan2 warp_sum2(scan2 v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        v.n += __shfl_down_sync(0xffffffffu, v.n, o);
+        v.e += __shfl_down_sync(0xffffffffu, v.e, o);
+    }
+    return v;
+}
+
+// pass 1: totals of every block's contiguous chunk [b * chunk, (b + 1) * chunk)
+__global__ void __launch_bounds__(SCAN_T) k_cscan_totals(pn_geom g, pn_ptrs P, long long chunk, scan2* part) {
+    __shared__ scan2 sm[32];
+    const long long lo = blockIdx.x * chunk, hi = min(lo + chunk, g.npad);
+    scan2 v{0ull, 0ull};
+    for (long long n = lo + threadIdx.x; n < hi; n += SCAN_T) v = v + node_counts(g, P, n);
+    v = warp_sum2(v);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = sm[threadIdx.x];
+        v = warp_sum2(v);
+        if (threadIdx.x == 0) part[blockIdx.x] = v;
+    }
+}
+
+// pass 2 (one block): exclusive scan of the block totals in place; grand totals -> state
+__global__ void __launch_bounds__(SCAN_T) k_cscan_partials(int nblocks, scan2* part, pn_state* st) {
+    if (threadIdx.x == 0) {
+        scan2 run{0ull, 0ull};
+        for (int b = 0; b < nblocks; ++b) { const scan2 t = part[b]; part[b] = run; run = run + t; }
+        st->cm = run.n;
+        st->clong = run.e;
+    }
+}
+
+// pass 3: lattice -> compact index (cidx, -1 on nodes that are not unknowns), compact -> lattice (lat); a long row's
+// third slot gets the code of its overflow record (-1 - record)
+__global__ void __launch_bounds__(SCAN_T) k_cscan_write(pn_geom g, pn_ptrs P, long long chunk, const scan2* part, int* cidx,
+                                                         int* lat, int* c2) {
+    __shared__ scan2 wsum[32];
+    __shared__ scan2 carry;
+    const long long lo = blockIdx.x * chunk, hi = min(lo + chunk, g.npad);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry = part[blockIdx.x];
+    __syncthreads();
+    for (long long base = lo; base < hi; base += SCAN_T) {
+        const long long n = base + threadIdx.x;
+        const scan2 mine = n < hi ? node_counts(g, P, n) : scan2{0ull, 0ull};
+        scan2 inc = mine;                                   // inclusive scan inside the warp
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long an = __shfl_up_sync(0xffffffffu, inc.n, o), ae = __shfl_up_sync(0xffffffffu, inc.e, o);
+            if (lane >= o) { inc.n += an; inc.e += ae; }
+        }
+        if (lane == 31) wsum[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {                                     // exclusive scan of the 32 warp totals
+            const scan2 t = wsum[lane];
+            scan2 s = t;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned long long an = __shfl_up_sync(0xffffffffu, s.n, o), ae = __shfl_up_sync(0xffffffffu, s.e, o);
+                if (lane >= o) { s.n += an; s.e += ae; }
+            }
+            wsum[lane] = scan2{s.n - t.n, s.e - t.e};
+        }
+        __syncthreads();
+        const scan2 c0 = carry, w0 = wsum[wid];
+        if (n < hi) {
+            const unsigned long long my_n = c0.n + w0.n + inc.n - mine.n, my_e = c0.e + w0.e + inc.e - mine.e;
+            if (mine.n) {
+                cidx[n] = (int)my_n;
+                lat[my_n] = (int)n;
+                c2[my_n] = mine.e ? -1 - (int)my_e : 0;
+            } else cidx[n] = -1;
+        }
+        __syncthreads();
+        if (threadIdx.x == SCAN_T - 1) carry = scan2{c0.n + w0.n + inc.n, c0.e + w0.e + inc.e};
+        __syncthreads();
+    }
+}
+
+// pass 4: the rows, neighbours in ascending compact order (-z, -y, -x, +x, +y, +z)
+__global__ void k_cfill(pn_geom g, pn_ptrs P, pn_cptrs C) {
+    const long long m = (long long)P.st->cm;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < m; i += (long long)gridDim.x * blockDim.x) {
+        const long long n = C.lat[i];
+        int ec[6];
+        float ev[6];
+        int k = 0;
+        float w;
+        w = P.w[2][n - g.plane]; if (w != 0.f) { ec[k] = C.cidx[n - g.plane]; ev[k] = w; ++k; }
+        w = P.w[1][n - g.px];    if (w != 0.f) { ec[k] = C.cidx[n - g.px];    ev[k] = w; ++k; }
+        w = P.w[0][n - 1];       if (w != 0.f) { ec[k] = C.cidx[n - 1];       ev[k] = w; ++k; }
+        w = P.w[0][n];           if (w != 0.f) { ec[k] = C.cidx[n + 1];       ev[k] = w; ++k; }
+        w = P.w[1][n];           if (w != 0.f) { ec[k] = C.cidx[n + g.px];    ev[k] = w; ++k; }
+        w = P.w[2][n];           if (w != 0.f) { ec[k] = C.cidx[n + g.plane]; ev[k] = w; ++k; }
+        for (int u = k; u < 6; ++u) { ec[u] = (int)i; ev[u] = 0.f; }   // unused slots: the row itself, weight 0
+        C.c[0][i] = ec[0]; C.v[0][i] = ev[0];
+        C.c[1][i] = ec[1]; C.v[1][i] = ev[1];
+        if (k <= 3) { C.c[2][i] = ec[2]; C.v[2][i] = ev[2]; }
+        else {
+            const int rec = -1 - C.c[2][i];               // written by k_cscan_write
+            C.v[2][i] = 0.f;
+            reinterpret_cast<int4*>(C.ovc)[rec] = make_int4(ec[2], ec[3], ec[4], ec[5]);
+            reinterpret_cast<float4*>(C.ovv)[rec] = make_float4(ev[2], ev[3], ev[4], ev[5]);
+        }
+    }
+}
+
+// ---- between the two numberings (once per fp64 residual replacement) -----------------------------------------------
+__global__ void k_cgather(pn_ptrs P, pn_cptrs C) {
+    const long long m = (long long)P.st->cm;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < m; i += (long long)gridDim.x * blockDim.x)
+        C.r[i] = P.r[C.lat[i]];
+}
+
+// S7 in the compact numbering: x64 += s (x_hat + alpha_x p) on the unknowns; x_hat = 0
+__global__ void k_cflush(pn_ptrs P, pn_cptrs C) {
+    const long long m = (long long)P.st->cm;
+    const double ax = P.st->alpha_x;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < m; i += (long long)gridDim.x * blockDim.x) {
+        const long long n = C.lat[i];
+        P.x64[n] += (double)P.s[n] * ((double)C.x[i] + ax * (double)C.p[i]);
+        C.x[i] = 0.f;
+    }
+}
+
+// ---- the iteration ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ void st4(float* p, const float4& v) { *reinterpret_cast<float4*>(p) = v; }
+
+// r_t = r - alpha q ; x_hat += alpha p ; p_t = r_t + beta p ; r_t.r_t -> state.part[0]   (alpha = alpha_{t-1}, 0 right
+// after a residual replacement; beta = beta_t, predicted by the previous k_cspmv or set from the true residual)
+__global__ void __launch_bounds__(TPB) k_cupdate(pn_ptrs P, pn_cptrs C) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;
+    __shared__ double sm[32];
+    __shared__ double tot[1];
+    const long long m = (long long)st->cm, m4 = m >> 2;
+    const float al = (float)st->alpha, nal = -al, beta = (float)st->beta;
+    double acc = 0.0;
+    for (long long v = blockIdx.x * (long long)blockDim.x + threadIdx.x; v < m4; v += (long long)gridDim.x * blockDim.x) {
+        const long long i = 4 * v;
+        float4 r = ld4(C.r + i);
+        const float4 q = __ldcs(reinterpret_cast<const float4*>(C.q + i));
+        float4 p = ld4(C.p + i), x = ld4(C.x + i);
+        r.x = fmaf(nal, q.x, r.x); r.y = fmaf(nal, q.y, r.y); r.z = fmaf(nal, q.z, r.z); r.w = fmaf(nal, q.w, r.w);
+        x.x = fmaf(al, p.x, x.x); x.y = fmaf(al, p.y, x.y); x.z = fmaf(al, p.z, x.z); x.w = fmaf(al, p.w, x.w);
+        p.x = fmaf(beta, p.x, r.x); p.y = fmaf(beta, p.y, r.y); p.z = fmaf(beta, p.z, r.z); p.w = fmaf(beta, p.w, r.w);
+        st4(C.r + i, r); st4(C.x + i, x); st4(C.p + i, p);
+        acc += (double)(r.x * r.x + r.y * r.y + r.z * r.z + r.w * r.w);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (int)(m - 4 * m4)) {   // the last 0..3 unknowns
+        const long long i = 4 * m4 + threadIdx.x;
+        const float r = fmaf(nal, C.q[i], C.r[i]);
+        const float p = C.p[i];
+        C.x[i] = fmaf(al, p, C.x[i]);
+        C.r[i] = r;
+        C.p[i] = fmaf(beta, p, r);
+        acc += (double)(r * r);
+    }
+    acc = pn_block_sum(acc, sm);
+    const double v1[1] = {acc};
+    if (pn_grid_sum<1>(v1, P.slots, &st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) st->part[0] = tot[0];
+    }
+}
+
+// q_t = p_t - W p_t over the table rows ; p.q, r.q, q.q ; last block: alpha_t, predicted beta_{t+1}, flags (pn_finish_F)
+__global__ void __launch_bounds__(TPB) k_cspmv(pn_ptrs P, pn_cptrs C) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;
+    __shared__ double sm[32];
+    __shared__ double tot[3];
+    const long long m = (long long)st->cm, m4 = m >> 2;
+    const float* __restrict__ p = C.p;
+    double a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
+    // one row: two dependent rounds of loads (slots, then the gathered p); FOUR consecutive rows per thread put four
+    // times as many of them in flight (measured on configs[2]: one row per thread ran at 2.4 TB/s, latency-bound)
+    for (long long v = blockIdx.x * (long long)blockDim.x + threadIdx.x; v < m4; v += (long long)gridDim.x * blockDim.x) {
+        const long long i = 4 * v;
+        const int4 c0 = *reinterpret_cast<const int4*>(C.c[0] + i), c1 = *reinterpret_cast<const int4*>(C.c[1] + i),
+                   c2 = *reinterpret_cast<const int4*>(C.c[2] + i);
+        const float4 v0 = ld4(C.v[0] + i), v1 = ld4(C.v[1] + i), v2 = ld4(C.v[2] + i);
+        const float4 pi = ld4(p + i), ri = ld4(C.r + i);
+        const int cc0[4] = {c0.x, c0.y, c0.z, c0.w}, cc1[4] = {c1.x, c1.y, c1.z, c1.w}, cc2[4] = {c2.x, c2.y, c2.z, c2.w};
+        const float w0[4] = {v0.x, v0.y, v0.z, v0.w}, w1[4] = {v1.x, v1.y, v1.z, v1.w}, w2[4] = {v2.x, v2.y, v2.z, v2.w};
+        const float pp[4] = {pi.x, pi.y, pi.z, pi.w};
+        float g0[4], g1[4], g2[4], qq[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            g0[u] = p[cc0[u]];
+            g1[u] = p[cc1[u]];
+            g2[u] = cc2[u] >= 0 ? p[cc2[u]] : 0.f;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float acc = w0[u] * g0[u];
+            acc = fmaf(w1[u], g1[u], acc);
+            if (cc2[u] >= 0) acc = fmaf(w2[u], g2[u], acc);
+            else {                                          // long row: entries 3..6 from its overflow record
+                const int4 oc = reinterpret_cast<const int4*>(C.ovc)[-1 - cc2[u]];
+                const float4 ov = reinterpret_cast<const float4*>(C.ovv)[-1 - cc2[u]];
+                acc = fmaf(ov.x, p[oc.x], acc);
+                acc = fmaf(ov.y, p[oc.y], acc);
+                acc = fmaf(ov.z, p[oc.z], acc);
+                acc = fmaf(ov.w, p[oc.w], acc);
+            }
+            qq[u] = pp[u] - acc;
+        }
+        const float4 q = make_float4(qq[0], qq[1], qq[2], qq[3]);
+        st4(C.q + i, q);
+        a_pq += (double)(pi.x * q.x + pi.y * q.y + pi.z * q.z + pi.w * q.w);
+        a_rq += (double)(ri.x * q.x + ri.y * q.y + ri.z * q.z + ri.w * q.w);
+        a_qq += (double)(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (int)(m - 4 * m4)) {   // the last 0..3 rows
+        const long long i = 4 * m4 + threadIdx.x;
+        const int c2 = C.c[2][i];
+        const float pi = p[i];
+        float acc = C.v[0][i] * p[C.c[0][i]];
+        acc = fmaf(C.v[1][i], p[C.c[1][i]], acc);
+        if (c2 >= 0) acc = fmaf(C.v[2][i], p[c2], acc);
+        else {
+            const int4 oc = reinterpret_cast<const int4*>(C.ovc)[-1 - c2];
+            const float4 ov = reinterpret_cast<const float4*>(C.ovv)[-1 - c2];
+            acc = fmaf(ov.x, p[oc.x], acc);
+            acc = fmaf(ov.y, p[oc.y], acc);
+            acc = fmaf(ov.z, p[oc.z], acc);
+            acc = fmaf(ov.w, p[oc.w], acc);
+        }
+        const float q = pi - acc;
+        C.q[i] = q;
+        a_pq += (double)(pi * q);
+        a_rq += (double)(C.r[i] * q);
+        a_qq += (double)(q * q);
+    }
+    a_pq = pn_block_sum(a_pq, sm);
+    a_rq = pn_block_sum(a_rq, sm);
+    a_qq = pn_block_sum(a_qq, sm);
+    const double v3[3] = {a_pq, a_rq, a_qq};
+    if (pn_grid_sum<3>(v3, P.slots, &st->ticket, sm, tot)) {
+        if (threadIdx.x == 0) pn_finish_F(st, st->part[0], tot[0], tot[1], tot[2]);
+    }
+}
+
+}  // namespace
+
+// Where the compact arrays live: in lattice-shaped arrays the structured kernels do not need during a compact solve.
+// Each holds npad floats; with `off` = cm rounded up to 64 entries and 2 * off <= npad, two row-indexed arrays share
+// one: p2 = c0 | c1, r2 = c2 | v0, q = v1 | v2, q2 = lat | overflow records (8 words per long row).  cidx is scratch of
+// the build only (P.r is rewritten by the first k_residual64 afterwards); the vectors q and r take the place of the
+// scaled weights, which the build has consumed by the time they are first written.
+bool pn_compact_fits(const pn_geom& g, long long m, long long n_long) {
+    const long long off = (m + 63) & ~63ll;
+    return m >= 1 && 2 * off <= g.npad && off + 8 * n_long + 8 <= g.npad;
+}
+
+pn_cptrs pn_compact_ptrs(const pn_ptrs& P, long long m, long long n_long) {
+    const long long off = (m + 63) & ~63ll;
+    pn_cptrs C;
+    C.cidx = (int*)P.r;
+    C.lat = (int*)P.q2;
+    C.ovc = (int*)P.q2 + off;
+    C.ovv = (float*)(C.ovc + 4 * ((n_long + 3) & ~3ll));
+    C.c[0] = (int*)P.p2; C.c[1] = (int*)P.p2 + off;
+    C.c[2] = (int*)P.r2; C.v[0] = P.r2 + off;
+    C.v[1] = P.q;        C.v[2] = P.q + off;
+    C.p = P.p;
+    C.x = P.xh;
+    C.q = P.w[0];
+    C.r = P.w[1];
+    return C;
+}
+
+static int scan_blocks(const pn_geom& g) {
+    int nb = g.sms * 8;
+    if (nb > PN_MAX_BLOCKS) nb = PN_MAX_BLOCKS;
+    const long long need = (g.npad + SCAN_T - 1) / SCAN_T;
+    if (nb > need) nb = (int)need;
+    return nb < 1 ? 1 : nb;
+}
+
+// passes 1-2: how many unknowns and long rows -> state.cm, state.clong (the host decides whether to compact)
+cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+    const int nb = scan_blocks(g);
+    const long long chunk = ((g.npad + nb - 1) / nb + SCAN_T - 1) / SCAN_T * SCAN_T;
+    scan2* part = reinterpret_cast<scan2*>(P.slots);
+    k_cscan_totals<<<nb, SCAN_T, 0, st>>>(g, P, chunk, part);
+    k_cscan_partials<<<1, SCAN_T, 0, st>>>(nb, part, P.st);
+    *launches += 2;
+    return cudaGetLastError();
+}
+
+// passes 3-4 (after pn_launch_compact_count, same scaled weights): numbering, table, zeroed q
+cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
+                                    int* launches) {
+    const int nb = scan_blocks(g);
+    const long long chunk = ((g.npad + nb - 1) / nb + SCAN_T - 1) / SCAN_T * SCAN_T;
+    k_cscan_write<<<nb, SCAN_T, 0, st>>>(g, P, chunk, reinterpret_cast<const scan2*>(P.slots), C.cidx, C.lat, C.c[2]);
+    k_cfill<<<grid_for(m, g.sms), TPB, 0, st>>>(g, P, C);
+    *launches += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return cudaMemsetAsync(C.q, 0, (size_t)m * 4, st);   // the weights' array becomes q (finite before its first use)
+}
+
+cudaError_t pn_launch_compact_gather(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
+                                     int* launches) {
+    k_cgather<<<grid_for(m, g.sms), TPB, 0, st>>>(P, C);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_compact_flush(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
+                                    int* launches) {
+    k_cflush<<<grid_for(m, g.sms), TPB, 0, st>>>(P, C);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+// `iterations` iterations of the compact scheme: two launches each
+cudaError_t pn_launch_compact_inner(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, int iterations, cudaStream_t st,
+                                    int* launches, cudaEvent_t* ev) {
+    int nb = g.sms * 8;
+    if (nb > PN_MAX_BLOCKS) nb = PN_MAX_BLOCKS;
+    if (ev) cudaEventRecord(ev[0], st);
+    for (int it = 0; it < iterations; ++it) {
+        k_cupdate<<<nb, TPB, 0, st>>>(P, C);
+        if (ev) cudaEventRecord(ev[2 * it + 1], st);
+        k_cspmv<<<nb, TPB, 0, st>>>(P, C);
+        if (ev) cudaEventRecord(ev[2 * it + 2], st);
+    }
+    *launches += 2 * iterations;
+    return cudaGetLastError();
+}

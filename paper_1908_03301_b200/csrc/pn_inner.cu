@@ -161,7 +161,7 @@ int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant) {
 // `scheme` is a resolved variant (1, 3 or 5).  ev (optional, 2*iterations+1 events): kernel boundaries, for
 // the per-kernel timing of PN_OPT_PROFILE (scheme 3: the second interval of every iteration is empty).
 cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int scheme, cudaStream_t st,
-                            int* launches, cudaEvent_t* ev) {
+                            int* launches, cudaEvent_t* ev, const pn_cptrs* compact) {
     const int nvec = (int)(g.npad / 4);
     const int nb = grid_for(nvec, g.sms);
     pn_fused_plan* fplan = nullptr;
@@ -173,6 +173,7 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
         *launches += 1;
         return e5;
     }
+    if (scheme == 7) return compact ? pn_launch_compact_inner(g, P, *compact, iterations, st, launches, ev) : cudaErrorInvalidValue;   // compacted unknowns (pn_compact.cu)
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];   // periodic lateral faces: k_wrap_fix finishes kernel A
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);

@@ -71,9 +71,12 @@ struct pn_state {
     double acc[4];              // results of the fp64 reductions (residual norms, b norm, flux)
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
     unsigned long long n_peeled;// solved nodes removed from the system as dangling ends (back-filled after the solve)
+    unsigned long long cm;      // active-node compaction (pn_compact.cu): unknowns of the inner system ...
+    unsigned long long clong;   // ... and rows of its neighbour table with more than three entries
     int flag;                   // 0 run, 1 proxy-converged, 2 reliable update due, 3 breakdown, 4 budget
     int iters;                  // inner iterations done in this solve
     int max_iters;
+    // bad_value, any_closed, topo_changed: cleared together (one memset of three ints), keep them adjacent
     int bad_value;              // set by the validation kernel
     int any_closed;             // some in-lattice bond has g == 0
     int topo_changed;           // pn_update_conductances / pn_replace_conductances: some bond went from closed to open or back
@@ -229,8 +232,9 @@ cudaError_t pn_launch_flush(const pn_geom& g, const pn_ptrs& P, int bufmode, cud
 cudaError_t pn_launch_set_state(const pn_ptrs& P, double rr, double beta, double rr_max, double rr_target,
                                 double delta2, int max_iters, int reset_iters, double xskip_min, cudaStream_t st,
                                 int* launches);
+struct pn_cptrs;
 cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, int variant, cudaStream_t st,
-                            int* launches, cudaEvent_t* ev);
+                            int* launches, cudaEvent_t* ev, const pn_cptrs* compact = nullptr);
 cudaError_t pn_launch_flux(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_dissipation(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_export_x(const pn_geom& g, const pn_ptrs& P, double* out, cudaStream_t st, int* launches);
@@ -254,6 +258,28 @@ bool pn_onchip_supported(const pn_geom& g);
 cudaError_t pn_fused_init_device();
 cudaError_t pn_onchip_init_device();
 cudaError_t pn_launch_cg_onchip(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st);
+
+// Active-node compaction (pn_compact.cu): the inner iteration on the unknowns only, ELL-3 + overflow neighbour table
+struct pn_cptrs {
+    int* cidx;                  // lattice -> compact index (build scratch)
+    int* lat;                   // compact -> lattice index
+    int* c[3];                  // three neighbour slots per row (compact numbering); c[2] < 0: -1 - overflow record
+    float* v[3];                // their scaled weights
+    int* ovc;                   // overflow records: entries 3..6 of the long rows, 4 indices ...
+    float* ovv;                 // ... and 4 weights per record
+    float *r, *q, *p, *x;       // cm entries each
+};
+bool pn_compact_fits(const pn_geom& g, long long m, long long n_long);
+pn_cptrs pn_compact_ptrs(const pn_ptrs& P, long long m, long long n_long);
+cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
+                                    int* launches);
+cudaError_t pn_launch_compact_gather(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
+                                     int* launches);
+cudaError_t pn_launch_compact_flush(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
+                                    int* launches);
+cudaError_t pn_launch_compact_inner(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, int iterations, cudaStream_t st,
+                                    int* launches, cudaEvent_t* ev);
 
 // Persistent in-place iteration for 2D lattices (pn_resident.cu): all iterations up to the next trigger in ONE cooperative launch
 bool pn_resident_supported(const pn_geom& g, const pn_ptrs& P);

@@ -777,3 +777,46 @@ def test_resident_scheme_fallbacks_and_budget(pn, oracle):
     a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: 6})
     b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: 6})
     assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]   # bit-reproducible
+
+
+# ---- active-node compaction (pn_compact.cu, kernel_scheme 7) ----
+@pytest.mark.parametrize("maker,direction", [
+    (lambda i: i.cfg3_percolation_3d(64, 64, 64), 0), (lambda i: i.cfg3_percolation_3d(40, 36, 33, p=0.32), 2),
+    (lambda i: i.cfg3_percolation_3d(66, 35, 33, p=0.29), 1), (lambda i: i.cfg3_percolation_3d(130, 30, 27, p=0.31), 0),
+    (lambda i: i.iid_diluted(257, 131, 1, seed=6, p=0.515), 1), (lambda i: i.iid_diluted(300, 520, 1, seed=8, p=0.51), 0)])
+def test_compacted_unknowns(pn, oracle, maker, direction):
+    """PN_OPT_COMPACT = 1 forces the CSR form wherever its table fits the workspace (at most one entry per padded lattice
+    node: networks near their threshold, 2D and 3D, ragged shapes, with and without peeling): pressures of ALL nodes,
+    classes and G_eff keep the parity bar; iteration counts stay those of the structured kernel to a few per cent (same
+    recurrences; the operator's sum is ordered differently)."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    # tol 1e-13: on these small near-threshold networks G_eff is carried by a few paths (1e-12 leaves ~2e-9 in it)
+    on, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3})
+    off, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 0, pn.PN_OPT_KERNEL: 3})
+    assert on.kernel_scheme == 7 and off.kernel_scheme == 3
+    assert on.n_unknowns == off.n_unknowns == on.n_solved - on.n_peeled
+    assert abs(on.inner_iters - off.inner_iters) <= 0.05 * off.inner_iters + 5
+    compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3, pn.PN_OPT_PEEL: 0,
+                                                         pn.PN_OPT_GRAPH: 0, pn.PN_OPT_CHUNK: 7, pn.PN_OPT_X0: 0})
+
+
+def test_compaction_policy_and_determinism(pn, oracle):
+    from paper_1908_03301_b200 import inputs
+    near = inputs.cfg3_percolation_3d(64, 64, 64)             # p = 0.30: a third of the nodes are unknowns after peeling
+    auto, *_ = compare(pn, oracle, near, 0)
+    assert auto.kernel_scheme == 7 and auto.n_unknowns < 0.45 * near.n_nodes
+    dense = inputs.cfg5_stratified_3d(32, 32, 32)
+    d, *_ = compare(pn, oracle, dense, 0)
+    assert d.kernel_scheme == 3                                # nothing to skip: the structured kernel
+    per, *_ = compare(pn, oracle, near, 0, periodic=True)
+    assert per.kernel_scheme == 3                              # periodic faces: the structured kernel + k_wrap_fix
+    forced, *_ = compare(pn, oracle, near, 0, opts={pn.PN_OPT_KERNEL: 3})
+    assert forced.kernel_scheme == 3                           # an explicit kernel choice is honoured
+    full, *_ = compare(pn, oracle, inputs.cfg4_fbm_cut_3d(48, 40, 36), 1, opts={pn.PN_OPT_COMPACT: 1})
+    assert full.kernel_scheme == 3                             # table larger than the workspace arrays: structured kernel
+    a = gpu_solve(pn, near, 0, 1e-10)
+    b = gpu_solve(pn, near, 0, 1e-10)
+    assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]
+    info, *_ = gpu_solve(pn, near, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40})
+    assert info.status == pn.PN_MAX_ITERS and info.kernel_scheme == 7 and 40 <= info.inner_iters <= 40 + 64
