@@ -31,8 +31,10 @@ def test_uniform_gives_linear_profile_and_gA_over_L(shape, direction):
     net = inputs.uniform(nx, ny, nz, g)
     res = run(net, direction)
     n_a = shape[direction]
-    coord = po._coord_along(nx, ny, nz, direction)[0]
-    expect = 1.0 - coord / (n_a - 1)
+    # P has shape (nz, ny, nx): the coordinate along lattice axis `direction` runs along array axis 2 - direction
+    shp = [1, 1, 1]
+    shp[2 - direction] = n_a
+    expect = np.broadcast_to(1.0 - np.arange(n_a, dtype=np.float64).reshape(shp) / (n_a - 1), (nz, ny, nx))
     assert np.max(np.abs(res.P - expect)) < 1e-12
     g32 = float(np.float32(g))
     s_perp = nx * ny * nz // n_a
