@@ -127,3 +127,45 @@ def test_c_oracle_periodic_matches_python_oracle(maker, direction):
     assert rel <= 1e-13 and pin == 0.0
     rel0, _ = c_oracle.certificate(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, a.P, direction)
     assert rel0 > 1e-6          # the no-flux operator rejects the periodic solution
+
+
+def test_starting_iterate_and_decade_log():
+    """`P_start` (used by tests/golden/make_digest.py to carry a tol-1e-12 solution on to the floor) changes only x0: the
+    continued solve lands on the zero-start solution; the per-decade iteration log is a record (monotone, ends at the
+    last decade reached) and does not touch the iteration."""
+    from oracle import c_oracle
+    from paper_1908_03301_b200 import inputs
+    net = inputs.cfg4_fbm_cut_3d(40, 36, 33)
+    args = (net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, 0)
+    zero = c_oracle.solve(*args, 1e-13)
+    a = c_oracle.solve(*args, 1e-12)
+    b = c_oracle.solve(*args, 1e-13, P_start=a.P)
+    assert a.status == b.status == zero.status == "ok"
+    assert 0 < b.iterations < 0.5 * zero.iterations
+    assert np.max(np.abs(b.P - zero.P)) <= 1e-9 and abs(b.g_eff - zero.g_eff) <= 1e-11 * abs(zero.g_eff)
+    assert np.array_equal(b.classes, zero.classes)
+    dec = [d for d in a.it_decade if d > 0]
+    assert dec == sorted(dec) and len(dec) == 13 and dec[-1] <= a.iterations    # decades 1e-0 .. 1e-12 reached
+    assert a.it_decade[13] == -1
+    c = c_oracle.solve(*args, 1e-12)
+    assert c.iterations == a.iterations and np.max(np.abs(c.P - a.P)) <= 1e-12      # (OpenMP sums: not bit-identical)
+
+
+def test_digest_script_on_a_small_sibling(tmp_path):
+    """tests/golden/make_digest.py end to end at 24^3: the stored numbers are the oracle's."""
+    import json
+    import os
+    import subprocess
+    import sys
+    from oracle import c_oracle
+    from paper_1908_03301_b200 import inputs
+    script = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "make_digest.py")
+    subprocess.check_call([sys.executable, script, "cfg4", "--n", "24", "--out", str(tmp_path)], stdout=subprocess.DEVNULL)
+    d = json.load(open(tmp_path / "cfg4_24_x_digest.json"))
+    sub = np.load(tmp_path / "cfg4_24_x_P_sub8.npy")
+    net = inputs.cfg4_fbm_cut_3d(24, 24, 24)
+    ref = c_oracle.solve(net.nx, net.ny, net.nz, net.gx, net.gy, net.gz, 0, 1e-13)
+    assert d["input_sha256"] == net.sha256() and d["n_solved"] == ref.n_solved
+    assert abs(d["g_eff"] - ref.g_eff) <= 1e-11 * abs(ref.g_eff)
+    assert np.max(np.abs(sub - ref.P[4::8, 4::8, 4::8])) <= 1e-9
+    assert len(d["plane_fluxes"]) == 23 and max(abs(f - d["g_eff"]) for f in d["plane_fluxes"]) <= 1e-9 * abs(d["g_eff"])
