@@ -184,20 +184,29 @@ k_cg_resident2d(pn_geom g, pn_ptrs P, int rows_max, int max_launch_iters) {
         if (lane == 0) { red[wid] = a_rr; red[32 + wid] = a_pq; red[64 + wid] = a_rq; red[96 + wid] = a_qq; }
         __syncthreads();
         if (wid == 0) {
+            // slot layout [parity][CTA][4]: one 32-byte sector per CTA
+            double* my = P.slots + ((size_t)pin * PN_MAX_BLOCKS + c) * 4;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const double v = pn_warp_sum(red[32 * k + lane]);
-                if (lane == 0) P.slots[(pin * 4 + k) * PN_MAX_BLOCKS + c] = v;
+                if (lane == 0) my[k] = v;
             }
             if (lane == 0) { bar_target += G; grid_barrier(bar, bar_target); }
             __syncwarp();
+            // all loads first (one round trip to L2), then the fixed-order sums: CTA b -> lane b % 32, ascending b per lane
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+            const double2* sl = reinterpret_cast<const double2*>(P.slots + (size_t)pin * PN_MAX_BLOCKS * 4);
+            double2 va[(PN_RESIDENT_MAX_CTAS + 31) / 32], vb[(PN_RESIDENT_MAX_CTAS + 31) / 32];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                double v = 0.0;
-                for (int b = lane; b < G; b += 32) v += __ldcg(P.slots + (pin * 4 + k) * PN_MAX_BLOCKS + b);
-                v = pn_warp_sum(v);
-                if (lane == 0) red[128 + k] = v;
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) {
+                const int b = lane + 32 * u;
+                va[u] = b < G ? __ldcg(sl + 2 * b) : make_double2(0.0, 0.0);
+                vb[u] = b < G ? __ldcg(sl + 2 * b + 1) : make_double2(0.0, 0.0);
             }
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) { t0 += va[u].x; t1 += va[u].y; t2 += vb[u].x; t3 += vb[u].y; }
+            t0 = pn_warp_sum(t0); t1 = pn_warp_sum(t1); t2 = pn_warp_sum(t2); t3 = pn_warp_sum(t3);
+            if (lane == 0) { red[128] = t0; red[129] = t1; red[130] = t2; red[131] = t3; }
             if (lane == 0) pn_finish_F(ls, red[128], red[129], red[130], red[131]);
         }
         __syncthreads();
