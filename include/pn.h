@@ -96,7 +96,7 @@ enum {
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
                                memory -- at most 7168 padded floats per array, no periodic faces --, 6 where it
-                               applies, else 3),
+                               applies, 1 on other lattices of at most 600 000 padded nodes, else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept as an independently written cross-check),
                                3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),

@@ -144,15 +144,23 @@ int grid_for(long long work_items, int sms) {
 
 }  // namespace
 
-// PN_OPT_KERNEL: 0 = automatic: the whole loop in one CTA when the lattice fits one SM's shared memory (5), else the
-// single fused TMA kernel at every size (3; measured on B200 with graph replay it is at least as fast as the reference
-// pair from 64^2 up, profiles/r01_small_lattices.md); 1 = reference two-kernel iteration (independently written
-// cross-check).  The two superseded schemes of round 1 (2: TMA S4 kernel + S5 kernel, 4: q recomputed) are gone;
-// their write-ups remain in profiles/r01_tma_kernel.md and profiles/r01_q_recompute_experiment.md.
-// 6 = persistent in-place kernel for 2D lattices up to 2048 wide (pn_resident.cu), the automatic choice where it applies.
+// PN_OPT_KERNEL: 0 = automatic: the whole loop in one CTA when the lattice fits one SM's shared memory (5); the persistent
+// shared-memory-resident kernel for 2D lattices whose slabs fit all SMs (6); the cache-fed pair below (1) for the other
+// lattices of at most PN_SMALL_LATTICE padded nodes; else the single fused TMA kernel (3).  Measured on B200 with BOTH
+// schemes replayed from CUDA graphs (profiles/r02_small_lattices.md; round 1's table had timed the pair without graph
+// replay): per iteration, pair / fused = 12.5 / 15.6 us at 64^3, 19.6 / 19.4 at 96^3, 26.1 / 26.1 at 128^3 -- the fused
+// kernel pays ~16 us of TMA ring ramp and reduction tail per launch, which only lattices from ~1 M nodes up amortise.
+// 1 = the pair on any lattice (independently written cross-check).  The two superseded schemes of round 1 (2: TMA S4
+// kernel + S5 kernel, 4: q recomputed) are gone; their write-ups remain in profiles/r01_tma_kernel.md and
+// profiles/r01_q_recompute_experiment.md.  6 = persistent in-place kernel for 2D lattices (pn_resident.cu).
+constexpr long long PN_SMALL_LATTICE = 600000;
 int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant) {
     const int big = pn_tma_supported() ? 3 : 1;
-    if (variant == 0) return pn_onchip_supported(g) ? 5 : (pn_resident_supported(g, P) ? 6 : big);
+    if (variant == 0) {
+        if (pn_onchip_supported(g)) return 5;
+        if (pn_resident_supported(g, P)) return 6;
+        return g.npad <= PN_SMALL_LATTICE ? 1 : big;
+    }
     if (variant == 5 && !pn_onchip_supported(g)) return big;   // too large for one SM, or periodic faces
     if (variant == 6 && !pn_resident_supported(g, P)) return big;   // 3D, wider than 2048, or periodic faces
     return variant;

@@ -684,7 +684,7 @@ def test_onchip_scheme_options(pn, oracle):
     on, *_ = compare(pn, oracle, net, 0, opts={pn.PN_OPT_PEEL: 1})
     assert on.n_peeled > 0 and on.kernel_scheme == 5
     per, *_ = compare(pn, oracle, net, 0, periodic=True)
-    assert per.kernel_scheme == 3                       # periodic faces: TMA kernel + k_wrap_fix
+    assert per.kernel_scheme == 1                       # periodic faces on a small lattice: the cache-fed pair + k_wrap_fix
     big, *_ = compare(pn, oracle, inputs.cfg3_percolation_3d(24, 24, 24, p=0.4), 0, opts={pn.PN_OPT_KERNEL: 5})
     assert big.kernel_scheme == 3                       # 24^3 does not fit: falls back
     a = gpu_solve(pn, net, 0, 1e-10)
@@ -808,15 +808,25 @@ def test_compaction_policy_and_determinism(pn, oracle):
     assert auto.kernel_scheme == 7 and auto.n_unknowns < 0.45 * near.n_nodes
     dense = inputs.cfg5_stratified_3d(32, 32, 32)
     d, *_ = compare(pn, oracle, dense, 0)
-    assert d.kernel_scheme == 3                                # nothing to skip: the structured kernel
+    assert d.kernel_scheme == 1                                # nothing to skip: a structured kernel (small lattice: the pair)
     per, *_ = compare(pn, oracle, near, 0, periodic=True)
-    assert per.kernel_scheme == 3                              # periodic faces: the structured kernel + k_wrap_fix
+    assert per.kernel_scheme == 1                              # periodic faces: a structured kernel + k_wrap_fix
     forced, *_ = compare(pn, oracle, near, 0, opts={pn.PN_OPT_KERNEL: 3})
     assert forced.kernel_scheme == 3                           # an explicit kernel choice is honoured
     full, *_ = compare(pn, oracle, inputs.cfg4_fbm_cut_3d(48, 40, 36), 1, opts={pn.PN_OPT_COMPACT: 1})
-    assert full.kernel_scheme == 3                             # table larger than the workspace arrays: structured kernel
+    assert full.kernel_scheme == 1                             # table larger than the workspace arrays: structured kernel
     a = gpu_solve(pn, near, 0, 1e-10)
     b = gpu_solve(pn, near, 0, 1e-10)
     assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]
     info, *_ = gpu_solve(pn, near, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40})
     assert info.status == pn.PN_MAX_ITERS and info.kernel_scheme == 7 and 40 <= info.inner_iters <= 40 + 64
+
+
+def test_automatic_kernel_choice_by_size(pn, oracle):
+    """0 = automatic: one CTA (5) / resident 2D slabs (6) / the cache-fed pair up to 600 000 padded nodes (1) / the fused TMA
+    kernel above (3) -- all through the same parity bar."""
+    from paper_1908_03301_b200 import inputs
+    for net, d, want in ((inputs.cfg5_stratified_3d(16, 16, 16), 0, 5), (inputs.cfg2_fbm_2d(300, 200), 0, 6),
+                         (inputs.cfg5_stratified_3d(64, 64, 64), 2, 1), (inputs.cfg5_stratified_3d(96, 96, 80), 0, 3)):
+        info, *_ = compare(pn, oracle, net, d)
+        assert info.kernel_scheme == want, (net.name, info.kernel_scheme)
