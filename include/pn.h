@@ -76,7 +76,9 @@ typedef struct {
                               they move 8 bytes per node less than the others                        */
     long long n_peeled;    /* solved nodes taken out of the system as dangling ends (PN_OPT_PEEL) and
                               back-filled after the solve; they are counted in n_solved too           */
-    long long n_unknowns;  /* unknowns of the inner linear system: n_solved - n_peeled                     */
+    long long n_unknowns;  /* unknowns of the inner linear system: n_solved - n_peeled - n_chain           */
+    long long n_chain;     /* solved nodes eliminated as links of degree-2 chains (PN_OPT_CONTRACT) and back-filled
+                              by interpolation between the ends of their chain; counted in n_solved too   */
     int labels_reused;     /* 1: S1's labelling and peeling were skipped, the classes of the previous solve
                               still hold (pn_update_conductances / pn_replace_conductances, no bond crossed zero) */
 } pn_info;
@@ -133,6 +135,13 @@ enum {
                                lattice nodes are unknowns (e.g. configs[2] after peeling: 0.33).  Applies to schemes
                                3 / 0 on lattices without periodic faces whose table fits the workspace; pressures of
                                all nodes are unchanged                                                        */
+    PN_OPT_CONTRACT = 13,   /* 1 (default): when the unknowns are compacted (PN_OPT_COMPACT), solved nodes with exactly two
+                               open bonds, both to solved nodes, are eliminated exactly beforehand -- a chain of them is
+                               one series resistor between its two end nodes (the Schur complement of the balance
+                               P:53) -- and take the resistance-weighted interpolation of the end pressures afterwards.
+                               Near the threshold these "links" are 69 % of the unknowns left after peeling and the
+                               reason for the slow convergence there.  0: never.  Pressures of all
+                               nodes stay those of the full system                                            */
     PN_OPT_XDEFER = 10      /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
                                iteration, two search directions at once (the earlier one recovered from p and r):
                                40 instead of 44 bytes per node-iteration on average; 0: every iteration    */

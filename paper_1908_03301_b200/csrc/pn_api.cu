@@ -40,6 +40,8 @@ struct pn_ctx {
     // node classes kept from the last solve (S8(f) item 4): reused while no bond crosses zero and nothing they depend on changes
     int reuse_labels;           // option
     int compact;                // option: active-node compaction 0 off, 1 on, 2 automatic
+    int contract;               // option: eliminate degree-2 chain nodes when compacting (pn_chain.cu)
+    int label_chains, label_compact, label_contract, label_variant;   // what the kept node classes were made with
     bool labels_valid, topo_dirty, warm_next;
     int label_dir, label_lateral, label_peel, label_skip;
     // CUDA graph of one chunk of inner iterations (captured on a private stream, launched on the caller's)
@@ -171,7 +173,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1; ctx->compact = 2;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1; ctx->compact = 2; ctx->contract = 1;
     ctx->delta = 0.3;   // measured: 0.3 needs 11 % fewer iterations than 0.1 on CFG2 2048^2 and the same on CFG3/4/5
     ctx->last_dir_user = -1;
     // per-handle device facts (no process-global state: handles on different devices are independent)
@@ -253,6 +255,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
+        case PN_OPT_CONTRACT: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->contract = (int)value; return PN_OK;
         case PN_OPT_COMPACT: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->compact = (int)value; return PN_OK;
         case PN_OPT_REUSE_LABELS: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->reuse_labels = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
@@ -398,9 +401,10 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     CK(cudaEventRecord(ctx->ev[0], s));
     // node classes of the previous solve still describe this network? (same direction and options, no bond crossed zero)
     const bool reuse = ctx->reuse_labels && ctx->labels_valid && !ctx->topo_dirty && ctx->label_dir == g.dir &&
-                       ctx->label_lateral == ctx->lateral && ctx->label_peel == ctx->peel && ctx->label_skip == ctx->skip_label;
+                       ctx->label_lateral == ctx->lateral && ctx->label_peel == ctx->peel && ctx->label_skip == ctx->skip_label &&
+                       ctx->label_compact == ctx->compact && ctx->label_contract == ctx->contract && ctx->label_variant == ctx->variant;
     ctx->labels_valid = false;   // until this solve's S1 has gone through
-    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + (reuse ? 0 : sizeof(P.st->count) + sizeof(P.st->n_peeled)), s));
+    CK(cudaMemsetAsync(P.st->acc, 0, sizeof(P.st->acc) + (reuse ? 0 : sizeof(P.st->count) + sizeof(P.st->n_peeled) + sizeof(P.st->n_chain)), s));
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     int scheme = pn_resolve_variant(g, P, ctx->variant);
@@ -436,11 +440,25 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
             CK(cudaMemsetAsync(&P.st->n_peeled, 0, sizeof(P.st->n_peeled), s));
         }
     }
-    CK(pn_launch_scale(g, P, s, &nl));
-    ctx->labels_valid = true;
-    ctx->topo_dirty = false;
-    ctx->warm_next = false;
-    ctx->label_dir = g.dir; ctx->label_lateral = ctx->lateral; ctx->label_peel = ctx->peel; ctx->label_skip = ctx->skip_label;
+    // active-node compaction may apply (decided below, once the scaled weights exist): automatic only with the automatic
+    // kernel choice -- an explicit PN_OPT_KERNEL is honoured unless PN_OPT_COMPACT = 1
+    const bool compact_allowed = (ctx->compact == 1 || (ctx->compact == 2 && ctx->variant == 0)) && !any_wrap && (scheme == 3 || scheme == 1);
+    // degree-2 chain nodes (pn_chain.cu) are eliminated together with the compaction: marked now, because the Jacobi scale
+    // and the weights of the reduced system depend on them
+    int chains = 0;
+    if (compact_allowed && ctx->contract && do_label) {
+        if (reuse) chains = ctx->label_chains;
+        else {
+            rc = read_state(ctx);
+            if (rc) return rc;
+            const double est = (double)ctx->h_state->count[0] - (double)ctx->h_state->n_peeled;
+            if (ctx->compact == 1 || est <= PN_COMPACT_MAX_FRACTION * (double)g.npad) {
+                CK(pn_launch_chain_mark(g, P, s, &nl));
+                chains = 1;
+            }
+        }
+    }
+    CK(pn_launch_scale(g, P, chains, s, &nl));
     // parent / flags aliased q / x_hat: clear the CG vectors before the first iteration
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
@@ -451,23 +469,33 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     CK(cudaMemsetAsync(P.p - g.plane, 0, vhalo, s));
     CK(cudaMemsetAsync(P.p2 - g.plane, 0, vhalo, s));
     // ---- active-node compaction (S8(f) item 1): when few lattice nodes are unknowns, iterate on the unknowns only ----
-    // 64 bytes per unknown and iteration against 40 per lattice node: automatic below 0.45 unknowns per padded node.  The
+    // 66 bytes per unknown and iteration against 40 per lattice node: automatic below 0.45 unknowns per padded node.  The
     // compact arrays live in lattice-shaped arrays (npad entries each): pn_compact_fits.
     long long cm = 0, clong = 0;
-    // (automatic only with the automatic kernel choice: an explicit PN_OPT_KERNEL is honoured unless PN_OPT_COMPACT = 1)
-    if ((ctx->compact == 1 || (ctx->compact == 2 && ctx->variant == 0)) && !any_wrap && (scheme == 3 || scheme == 1)) {
-        CK(pn_launch_compact_count(g, P, s, &nl));
+    if (compact_allowed) {
+        CK(pn_launch_compact_count(g, P, chains, s, &nl));
         rc = read_state(ctx);
         if (rc) return rc;
         const long long m = (long long)ctx->h_state->cm, nl_rows = (long long)ctx->h_state->clong;
         const bool want = ctx->compact == 1 || (double)m <= PN_COMPACT_MAX_FRACTION * (double)g.npad;
         if (want && pn_compact_fits(g, m, nl_rows)) {
             ctx->C = pn_compact_ptrs(P, m, nl_rows);
-            CK(pn_launch_compact_build(g, P, ctx->C, m, s, &nl));
+            CK(pn_launch_compact_build(g, P, ctx->C, m, chains, s, &nl));
             cm = m; clong = nl_rows;
             scheme = 7; fused = 1; bufmode = 2;
+        } else if (chains) {   // no compaction after all: the structured kernels need every solved node as an unknown again
+            CK(pn_launch_chain_unmark(g, P, s, &nl));
+            CK(cudaMemsetAsync(&P.st->n_chain, 0, sizeof(P.st->n_chain), s));
+            chains = 0;
+            CK(pn_launch_scale(g, P, 0, s, &nl));
         }
     }
+    ctx->labels_valid = true;
+    ctx->topo_dirty = false;
+    ctx->warm_next = false;
+    ctx->label_dir = g.dir; ctx->label_lateral = ctx->lateral; ctx->label_peel = ctx->peel; ctx->label_skip = ctx->skip_label;
+    ctx->label_chains = chains; ctx->label_compact = ctx->compact; ctx->label_contract = ctx->contract; ctx->label_variant = ctx->variant;
+    if (chains) CK(pn_launch_chain_fill(g, P, s, &nl));   // chain nodes follow the starting pressures of their chains' ends
     CK(pn_launch_residual64(g, P, bufmode, s, &nl));
     if (cm) CK(pn_launch_compact_gather(g, P, ctx->C, cm, s, &nl));
     CK(cudaEventRecord(ctx->ev[1], s));
@@ -558,6 +586,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
             const int flag = h->flag;
             if (cm) CK(pn_launch_compact_flush(g, P, ctx->C, cm, s, &nl));
             else CK(pn_launch_flush(g, P, bufmode, s, &nl));
+            if (chains) CK(pn_launch_chain_fill(g, P, s, &nl));
             CK(pn_launch_residual64(g, P, bufmode, s, &nl));
             if (cm) CK(pn_launch_compact_gather(g, P, ctx->C, cm, s, &nl));
             rc = read_state(ctx);
@@ -577,6 +606,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
             CK(pn_launch_set_state(P, rr_hat, beta, rr_hat, target_for(rn, rr_hat), delta2, ctx->max_iters, 0, xskip_min, s, &nl));
         }
     }
+    // (the last k_chain_fill ran before the last residual evaluation: the chain nodes are up to date)
     if (n_peeled > 0) CK(pn_launch_backfill(g, P, s, &nl));   // dangling ends take the pressure of the node they hang from
     CK(cudaEventRecord(ctx->ev[2], s));
     CK(cudaStreamSynchronize(s));
@@ -599,6 +629,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         info->n_peeled = n_peeled;
         info->labels_reused = reuse ? 1 : 0;
         info->n_unknowns = cm ? cm : n_solved - n_peeled;
+        info->n_chain = (long long)h->n_chain;
         if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
         if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
         info->t_stencil_ms = t_stencil;

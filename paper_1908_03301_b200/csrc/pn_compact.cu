@@ -21,7 +21,7 @@
 // adjacent and y / z neighbours a fixed few thousand entries away: the gathers are served by L1 / L2.
 // The fp64 outer steps stay on the lattice (k_residual64 writes r_hat there); k_cgather / k_cflush move r_hat and the
 // correction between the two numberings.  No periodic faces (those lattices keep the structured kernels).
-#include "pn_internal.cuh"
+#include "pn_chain.cuh"
 
 namespace {
 
@@ -41,15 +41,30 @@ int grid_for(long long work_items, int sms) {
 struct scan2 { unsigned long long n, e; };
 __device__ __forceinline__ scan2 operator+(const scan2& a, const scan2& b) { return scan2{a.n + b.n, a.e + b.e}; }
 
-// (is unknown, is a long row) of lattice node n: an unknown has a non-zero Jacobi scale; a table entry per non-zero
-// scaled weight (weights towards Dirichlet, pinned and peeled nodes are zero: they live in the diagonal and in b);
-// long = more than three entries
-__device__ __forceinline__ scan2 node_counts(const pn_geom& g, const pn_ptrs& P, long long n) {
+// scaled weight of the bond of padded node n in direction code c (0:+x 1:-x 2:+y 3:-y 4:+z 5:-z)
+__device__ __forceinline__ float weight_dir(const pn_geom& g, const pn_ptrs& P, long long n, int c) {
+    const int b = c >> 1;
+    const long long sb = b == 0 ? 1 : (b == 1 ? (long long)g.px : g.plane);
+    return P.w[b][(c & 1) ? n - sb : n];
+}
+// does direction c of unknown n give a table entry?  A non-zero scaled weight (weights towards Dirichlet, pinned and
+// peeled nodes are zero: they live in the diagonal and in b), or -- with degree-2 chains eliminated (pn_chain.cu) -- an
+// open bond towards a chain node: the entry then points at the chain's far end
+__device__ __forceinline__ bool has_entry(const pn_geom& g, const pn_ptrs& P, long long n, int c, int chains) {
+    if (weight_dir(g, P, n, c) != 0.f) return true;
+    if (!chains) return false;
+    long long m;
+    return pn_bond_dir(g, P, n, c, &m) != 0.f && P.cls[m] == PN_CLASS_CHAIN;
+}
+
+// (is unknown, is a long row) of lattice node n: an unknown has a non-zero Jacobi scale; long = more than three entries
+__device__ __forceinline__ scan2 node_counts(const pn_geom& g, const pn_ptrs& P, long long n, int chains) {
     scan2 v{0ull, 0ull};
     if (P.s[n] != 0.f) {
         v.n = 1ull;
-        const int deg = (P.w[2][n - g.plane] != 0.f) + (P.w[1][n - g.px] != 0.f) + (P.w[0][n - 1] != 0.f) +
-                        (P.w[0][n] != 0.f) + (P.w[1][n] != 0.f) + (P.w[2][n] != 0.f);
+        int deg = 0;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) deg += has_entry(g, P, n, c, chains) ? 1 : 0;
         v.e = deg > 3 ? 1ull : 0ull;
     }
     return v;
@@ -65,11 +80,11 @@ __device__ __forceinline__ scan2 warp_sum2(scan2 v) {
 }
 
 // pass 1: totals of every block's contiguous chunk [b * chunk, (b + 1) * chunk)
-__global__ void __launch_bounds__(SCAN_T) k_cscan_totals(pn_geom g, pn_ptrs P, long long chunk, scan2* part) {
+__global__ void __launch_bounds__(SCAN_T) k_cscan_totals(pn_geom g, pn_ptrs P, int chains, long long chunk, scan2* part) {
     __shared__ scan2 sm[32];
     const long long lo = blockIdx.x * chunk, hi = min(lo + chunk, g.npad);
     scan2 v{0ull, 0ull};
-    for (long long n = lo + threadIdx.x; n < hi; n += SCAN_T) v = v + node_counts(g, P, n);
+    for (long long n = lo + threadIdx.x; n < hi; n += SCAN_T) v = v + node_counts(g, P, n, chains);
     v = warp_sum2(v);
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
     __syncthreads();
@@ -92,8 +107,8 @@ __global__ void __launch_bounds__(SCAN_T) k_cscan_partials(int nblocks, scan2* p
 
 // pass 3: lattice -> compact index (cidx, -1 on nodes that are not unknowns), compact -> lattice (lat); a long row's
 // third slot gets the code of its overflow record (-1 - record)
-__global__ void __launch_bounds__(SCAN_T) k_cscan_write(pn_geom g, pn_ptrs P, long long chunk, const scan2* part, int* cidx,
-                                                         int* lat, int* c2) {
+__global__ void __launch_bounds__(SCAN_T) k_cscan_write(pn_geom g, pn_ptrs P, int chains, long long chunk, const scan2* part,
+                                                         int* cidx, int* lat, int* c2) {
     __shared__ scan2 wsum[32];
     __shared__ scan2 carry;
     const long long lo = blockIdx.x * chunk, hi = min(lo + chunk, g.npad);
@@ -102,7 +117,7 @@ __global__ void __launch_bounds__(SCAN_T) k_cscan_write(pn_geom g, pn_ptrs P, lo
     __syncthreads();
     for (long long base = lo; base < hi; base += SCAN_T) {
         const long long n = base + threadIdx.x;
-        const scan2 mine = n < hi ? node_counts(g, P, n) : scan2{0ull, 0ull};
+        const scan2 mine = n < hi ? node_counts(g, P, n, chains) : scan2{0ull, 0ull};
         scan2 inc = mine;                                   // inclusive scan inside the warp
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -137,21 +152,32 @@ __global__ void __launch_bounds__(SCAN_T) k_cscan_write(pn_geom g, pn_ptrs P, lo
     }
 }
 
-// pass 4: the rows, neighbours in ascending compact order (-z, -y, -x, +x, +y, +z)
-__global__ void k_cfill(pn_geom g, pn_ptrs P, pn_cptrs C) {
+// pass 4: the rows, directions in the order -z, -y, -x, +x, +y, +z (ascending compact index without chains).  With
+// chains eliminated a bond towards a chain node becomes the entry (far end of the chain, series conductance x the two
+// Jacobi scales), rounded once from fp64 like every weight; a chain that loops back to the row itself carries no current
+// and leaves an empty slot.  Parallel entries (two chains, or a chain and a bond, to the same node) stay separate.
+__global__ void k_cfill(pn_geom g, pn_ptrs P, pn_cptrs C, int chains) {
     const long long m = (long long)P.st->cm;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < m; i += (long long)gridDim.x * blockDim.x) {
         const long long n = C.lat[i];
         int ec[6];
         float ev[6];
         int k = 0;
-        float w;
-        w = P.w[2][n - g.plane]; if (w != 0.f) { ec[k] = C.cidx[n - g.plane]; ev[k] = w; ++k; }
-        w = P.w[1][n - g.px];    if (w != 0.f) { ec[k] = C.cidx[n - g.px];    ev[k] = w; ++k; }
-        w = P.w[0][n - 1];       if (w != 0.f) { ec[k] = C.cidx[n - 1];       ev[k] = w; ++k; }
-        w = P.w[0][n];           if (w != 0.f) { ec[k] = C.cidx[n + 1];       ev[k] = w; ++k; }
-        w = P.w[1][n];           if (w != 0.f) { ec[k] = C.cidx[n + g.px];    ev[k] = w; ++k; }
-        w = P.w[2][n];           if (w != 0.f) { ec[k] = C.cidx[n + g.plane]; ev[k] = w; ++k; }
+        const int order[6] = {5, 3, 1, 0, 2, 4};
+#pragma unroll 1
+        for (int o = 0; o < 6; ++o) {
+            const int c = order[o];
+            const float w = weight_dir(g, P, n, c);
+            long long mnode;
+            const float gv = pn_bond_dir(g, P, n, c, &mnode);
+            if (w != 0.f) { ec[k] = C.cidx[mnode]; ev[k] = w; ++k; }
+            else if (chains && gv != 0.f && P.cls[mnode] == PN_CLASS_CHAIN) {
+                const pn_walk wk = pn_chain_canonical(g, P, n, c);
+                if (wk.end == n) { ec[k] = (int)i; ev[k] = 0.f; }
+                else { ec[k] = C.cidx[wk.end]; ev[k] = (float)((1.0 / wk.R) * (double)P.s[n] * (double)P.s[wk.end]); }
+                ++k;
+            }
+        }
         for (int u = k; u < 6; ++u) { ec[u] = (int)i; ev[u] = 0.f; }   // unused slots: the row itself, weight 0
         C.c[0][i] = ec[0]; C.v[0][i] = ev[0];
         C.c[1][i] = ec[1]; C.v[1][i] = ev[1];
@@ -340,23 +366,23 @@ static int scan_blocks(const pn_geom& g) {
 }
 
 // passes 1-2: how many unknowns and long rows -> state.cm, state.clong (the host decides whether to compact)
-cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, int chains, cudaStream_t st, int* launches) {
     const int nb = scan_blocks(g);
     const long long chunk = ((g.npad + nb - 1) / nb + SCAN_T - 1) / SCAN_T * SCAN_T;
     scan2* part = reinterpret_cast<scan2*>(P.slots);
-    k_cscan_totals<<<nb, SCAN_T, 0, st>>>(g, P, chunk, part);
+    k_cscan_totals<<<nb, SCAN_T, 0, st>>>(g, P, chains, chunk, part);
     k_cscan_partials<<<1, SCAN_T, 0, st>>>(nb, part, P.st);
     *launches += 2;
     return cudaGetLastError();
 }
 
 // passes 3-4 (after pn_launch_compact_count, same scaled weights): numbering, table, zeroed q
-cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
-                                    int* launches) {
+cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, int chains,
+                                    cudaStream_t st, int* launches) {
     const int nb = scan_blocks(g);
     const long long chunk = ((g.npad + nb - 1) / nb + SCAN_T - 1) / SCAN_T * SCAN_T;
-    k_cscan_write<<<nb, SCAN_T, 0, st>>>(g, P, chunk, reinterpret_cast<const scan2*>(P.slots), C.cidx, C.lat, C.c[2]);
-    k_cfill<<<grid_for(m, g.sms), TPB, 0, st>>>(g, P, C);
+    k_cscan_write<<<nb, SCAN_T, 0, st>>>(g, P, chains, chunk, reinterpret_cast<const scan2*>(P.slots), C.cidx, C.lat, C.c[2]);
+    k_cfill<<<grid_for(m, g.sms), TPB, 0, st>>>(g, P, C, chains);
     *launches += 2;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

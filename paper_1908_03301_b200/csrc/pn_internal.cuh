@@ -71,6 +71,7 @@ struct pn_state {
     double acc[4];              // results of the fp64 reductions (residual norms, b norm, flux)
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
     unsigned long long n_peeled;// solved nodes removed from the system as dangling ends (back-filled after the solve)
+    unsigned long long n_chain; // solved nodes eliminated as links of degree-2 chains (pn_chain.cu; back-filled)
     unsigned long long cm;      // active-node compaction (pn_compact.cu): unknowns of the inner system ...
     unsigned long long clong;   // ... and rows of its neighbour table with more than three entries
     int flag;                   // 0 run, 1 proxy-converged, 2 reliable update due, 3 breakdown, 4 budget
@@ -222,7 +223,7 @@ cudaError_t pn_launch_update_raw(int unx, int uny, int unz, const pn_ptrs& P, fl
                                  int* launches);
 cudaError_t pn_launch_replace_raw(const pn_geom& g, float* raw, const float* src, int axis_internal, pn_state* state,
                                   cudaStream_t st, int* launches);
-cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, int chains, cudaStream_t st, int* launches);
 cudaError_t pn_launch_unpeel(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_backfill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 // `bufmode`: which buffers hold the vectors of the inner iteration -- 0: two-kernel schemes (r single, p double-buffered
@@ -259,6 +260,12 @@ cudaError_t pn_fused_init_device();
 cudaError_t pn_onchip_init_device();
 cudaError_t pn_launch_cg_onchip(const pn_geom& g, const pn_ptrs& P, int max_launch_iters, cudaStream_t st);
 
+// Degree-2 chain elimination (pn_chain.cu): mark / undo, reduced Jacobi scale, back-fill by interpolation
+cudaError_t pn_launch_chain_mark(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+cudaError_t pn_launch_chain_unmark(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+cudaError_t pn_launch_chain_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+cudaError_t pn_launch_chain_fill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+
 // Active-node compaction (pn_compact.cu): the inner iteration on the unknowns only, ELL-3 + overflow neighbour table
 struct pn_cptrs {
     int* cidx;                  // lattice -> compact index (build scratch)
@@ -271,9 +278,10 @@ struct pn_cptrs {
 };
 bool pn_compact_fits(const pn_geom& g, long long m, long long n_long);
 pn_cptrs pn_compact_ptrs(const pn_ptrs& P, long long m, long long n_long);
-cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
-cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
-                                    int* launches);
+// `chains`: degree-2 chain nodes are marked (pn_chain.cu): a bond towards one is a table entry to the chain's far end
+cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, int chains, cudaStream_t st, int* launches);
+cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, int chains,
+                                    cudaStream_t st, int* launches);
 cudaError_t pn_launch_compact_gather(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,
                                      int* launches);
 cudaError_t pn_launch_compact_flush(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, cudaStream_t st,

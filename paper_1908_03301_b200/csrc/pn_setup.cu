@@ -7,7 +7,7 @@
 // follow SURVEY.md 8(c) steps 2-3.  The labelling is a lock-free union-find over the interior nodes
 // (hook the larger root under the smaller with atomicCAS, path halving on find); the oracle uses a
 // serial BFS, so the two share nothing but the definition of a component.
-#include "pn_internal.cuh"
+#include "pn_chain.cuh"
 
 namespace {
 
@@ -337,13 +337,14 @@ __global__ void k_prune(pn_geom g, pn_ptrs P) {
     const long long stride[3] = {1, g.px, g.plane};
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const int c0 = P.cls[n];
-        const bool keep0 = c0 <= PN_CLASS_SOLVED;
+        const bool keep0 = c0 <= PN_CLASS_SOLVED || c0 == PN_CLASS_CHAIN;   // (chain nodes: label reuse; they keep their bonds)
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
             const float v = P.gs[b][n];
             if (v == 0.f) continue;
             // v != 0 implies the forward neighbour is a real node (off-lattice entries were zeroed)
-            const bool keep1 = P.cls[n + stride[b]] <= PN_CLASS_SOLVED;
+            const int c1 = P.cls[n + stride[b]];
+            const bool keep1 = c1 <= PN_CLASS_SOLVED || c1 == PN_CLASS_CHAIN;
             if (!(keep0 && keep1)) P.gs[b][n] = 0.f;
         }
     }
@@ -414,7 +415,7 @@ __global__ void k_peel(pn_geom g, pn_ptrs P) {
 __global__ void k_unpeel(pn_geom g, pn_ptrs P) {
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const int c = P.cls[n];
-        if (c < PN_CLASS_PEELED) continue;
+        if (c < PN_CLASS_PEELED || c >= PN_CLASS_CHAIN) continue;
         const int code = c - PN_CLASS_PEELED, b = code >> 1, side = code & 1;
         const pn_nb nb = pn_nbr(g, P, n, coords_of(g, n), b, side);
         const coords cc = coords_of(g, side == 0 ? n : nb.m);      // the node whose FORWARD entry this bond is
@@ -427,9 +428,9 @@ __global__ void k_unpeel(pn_geom g, pn_ptrs P) {
 __global__ void k_backfill(pn_geom g, pn_ptrs P) {
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         int c = P.cls[n];
-        if (c < PN_CLASS_PEELED) continue;
+        if (c < PN_CLASS_PEELED || c >= PN_CLASS_CHAIN) continue;
         long long m = n;
-        for (long long guard = 0; c >= PN_CLASS_PEELED && guard < g.npad; ++guard) {
+        for (long long guard = 0; c >= PN_CLASS_PEELED && c < PN_CLASS_CHAIN && guard < g.npad; ++guard) {
             const int code = c - PN_CLASS_PEELED;
             m = pn_nbr(g, P, m, coords_of(g, m), code >> 1, code & 1).m;
             c = P.cls[m];
@@ -554,9 +555,13 @@ cudaError_t pn_launch_replace_raw(const pn_geom& g, float* raw, const float* src
 }
 
 // Diagonal scale, ||b||^2 and the scaled weights of the inner system, from the final solve copy.
-cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
+cudaError_t pn_launch_scale(const pn_geom& g, const pn_ptrs& P, int chains, cudaStream_t st, int* launches) {
     const int nb = grid_for(g.npad, g.sms);
     k_scale<<<nb, TPB, 0, st>>>(g, P);
+    if (chains) {   // the nodes next to a chain take the reduced system's diagonal before the weights are formed
+        cudaError_t e = pn_launch_chain_scale(g, P, st, launches);
+        if (e != cudaSuccess) return e;
+    }
     k_weights<<<nb, TPB, 0, st>>>(g, P);
     *launches += 2;
     if (g.wrap[0] || g.wrap[1] || g.wrap[2]) {

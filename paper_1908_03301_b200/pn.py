@@ -24,7 +24,7 @@ LIB_PATH = os.path.join(HERE, "libpn.so")
 PN_OK, PN_NO_SPANNING_CLUSTER, PN_MAX_ITERS = 0, 1, 2
 PN_ERR_ARG, PN_ERR_STATE, PN_ERR_VALUE, PN_ERR_WORKSPACE, PN_ERR_CUDA, PN_ERR_BREAKDOWN = -1, -2, -3, -4, -5, -6
 (PN_OPT_MAX_ITERS, PN_OPT_DELTA, PN_OPT_X0, PN_OPT_CHUNK, PN_OPT_SKIP_LABEL, PN_OPT_KERNEL, PN_OPT_PROFILE,
- PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER, PN_OPT_REUSE_LABELS, PN_OPT_COMPACT) = range(13)
+ PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER, PN_OPT_REUSE_LABELS, PN_OPT_COMPACT, PN_OPT_CONTRACT) = range(14)
 CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CLASS_FLOATING = range(6)
 
 # every symbol include/pn.h declares (tests check that the library exports each of them)
@@ -43,7 +43,7 @@ class PnInfo(ctypes.Structure):
                 ("t_stencil_ms", ctypes.c_double), ("t_update_ms", ctypes.c_double),
                 ("n_timed_iters", ctypes.c_int), ("n_xskip", ctypes.c_int),
                 ("n_peeled", ctypes.c_longlong), ("n_unknowns", ctypes.c_longlong),
-                ("labels_reused", ctypes.c_int)]
+                ("n_chain", ctypes.c_longlong), ("labels_reused", ctypes.c_int)]
 
 
 @dataclass
@@ -67,6 +67,7 @@ class SolveInfo:
     n_xskip: int = 0
     labels_reused: int = 0
     n_unknowns: int = 0
+    n_chain: int = 0
 
 
 class PnError(RuntimeError):
@@ -240,7 +241,7 @@ class Network:
         return SolveInfo(rc, info.outer_cycles, info.inner_iters, info.rel_residual, info.b_norm, info.n_solved,
                          info.n_inlet_only, info.n_outlet_only, info.n_floating, info.t_label_ms, info.t_solve_ms,
                          info.t_stencil_ms, info.t_update_ms, info.n_timed_iters, info.kernel_scheme, info.n_peeled, info.n_xskip,
-                         info.labels_reused, info.n_unknowns)
+                         info.labels_reused, info.n_unknowns, info.n_chain)
 
     def pressures(self, out=None):
         """fp64 pressures on all nodes as a CUDA tensor of shape (nz, ny, nx)."""

@@ -792,13 +792,14 @@ def test_compacted_unknowns(pn, oracle, maker, direction):
     from paper_1908_03301_b200 import inputs
     net = maker(inputs)
     # tol 1e-13: on these small near-threshold networks G_eff is carried by a few paths (1e-12 leaves ~2e-9 in it)
-    on, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3})
+    on, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3, pn.PN_OPT_CONTRACT: 0})
     off, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 0, pn.PN_OPT_KERNEL: 3})
     assert on.kernel_scheme == 7 and off.kernel_scheme == 3
     assert on.n_unknowns == off.n_unknowns == on.n_solved - on.n_peeled
     assert abs(on.inner_iters - off.inner_iters) <= 0.05 * off.inner_iters + 5
     compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3, pn.PN_OPT_PEEL: 0,
-                                                         pn.PN_OPT_GRAPH: 0, pn.PN_OPT_CHUNK: 7, pn.PN_OPT_X0: 0})
+                                                         pn.PN_OPT_GRAPH: 0, pn.PN_OPT_CHUNK: 7, pn.PN_OPT_X0: 0,
+                                                         pn.PN_OPT_CONTRACT: 0})
 
 
 def test_compaction_policy_and_determinism(pn, oracle):
@@ -830,3 +831,60 @@ def test_automatic_kernel_choice_by_size(pn, oracle):
                          (inputs.cfg5_stratified_3d(64, 64, 64), 2, 1), (inputs.cfg5_stratified_3d(96, 96, 80), 0, 3)):
         info, *_ = compare(pn, oracle, net, d)
         assert info.kernel_scheme == want, (net.name, info.kernel_scheme)
+
+
+# ---- degree-2 chain elimination on top of the compacted unknowns (pn_chain.cu, PN_OPT_CONTRACT) ----
+@pytest.mark.parametrize("maker,direction", [
+    (lambda i: i.cfg3_percolation_3d(64, 64, 64), 0), (lambda i: i.cfg3_percolation_3d(40, 36, 33, p=0.32), 2),
+    (lambda i: i.cfg3_percolation_3d(66, 35, 33, p=0.29), 1), (lambda i: i.cfg3_percolation_3d(130, 30, 27, p=0.31), 0),
+    (lambda i: i.iid_diluted(257, 131, 1, seed=6, p=0.515), 1), (lambda i: i.iid_diluted(300, 520, 1, seed=8, p=0.51), 0),
+    (lambda i: i.iid_diluted(300, 520, 1, seed=9, p=0.52), 1)])
+def test_chain_elimination(pn, oracle, maker, direction):
+    """Links (solved nodes with two open bonds, both to solved nodes) are eliminated as series resistors and back-filled by
+    interpolation: pressures of ALL nodes, classes and G_eff keep the parity bar, with and without peeling (without it
+    dangling trees hang from chain nodes), from a zero start, and bit-reproducibly."""
+    from paper_1908_03301_b200 import inputs
+    net = maker(inputs)
+    base = {pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3}
+    on, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={**base, pn.PN_OPT_CONTRACT: 1})
+    off, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={**base, pn.PN_OPT_CONTRACT: 0})
+    assert on.kernel_scheme == 7 and off.kernel_scheme == 7
+    assert on.n_chain > 0 and off.n_chain == 0
+    assert on.n_unknowns == on.n_solved - on.n_peeled - on.n_chain and off.n_unknowns == on.n_unknowns + on.n_chain
+    assert on.inner_iters <= off.inner_iters
+    nopeel, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={**base, pn.PN_OPT_PEEL: 0, pn.PN_OPT_X0: 0, pn.PN_OPT_GRAPH: 0})
+    # (without peeling the table may outgrow the workspace arrays: then the marks are undone and the structured kernel runs)
+    assert nopeel.n_peeled == 0 and (nopeel.n_chain > 0 if nopeel.kernel_scheme == 7 else nopeel.n_chain == 0)
+    a = gpu_solve(pn, net, direction, 1e-10, opts=base)
+    b = gpu_solve(pn, net, direction, 1e-10, opts=base)
+    assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]
+
+
+def test_chain_elimination_hand_built(pn, oracle):
+    """A ladder whose rungs are mostly closed: long chains, a loop hanging from one node (closed ring of links), two chains
+    between the same pair of nodes (parallel entries), a chain next to a direct bond."""
+    nx, ny = 40, 6
+    gx = np.zeros((1, ny, nx), np.float32)
+    gy = np.zeros((1, ny, nx), np.float32)
+    rng = np.random.default_rng(1)
+    gx[0, 0, :] = rng.uniform(0.2, 2.0, nx)          # rail 0
+    gx[0, 1, :] = rng.uniform(0.2, 2.0, nx)          # rail 1
+    for i in (5, 6, 20, 33):                          # rungs between the rails (5, 6 adjacent: a 4-node loop of two chains)
+        gy[0, 0, i] = rng.uniform(0.2, 2.0)
+    # a ring hanging from rail 1 at i = 12: up along y to row 3, across to i = 15, back down
+    for j in (1, 2):
+        gy[0, j, 12] = 0.7
+        gy[0, j, 15] = 0.9
+    gx[0, 3, 12:15] = 1.1
+    # a stem from rail 1 at i = 25 up to (25, 3), which carries a closed ring of three links: a chain that loops back to its
+    # own end node (no current; all its nodes sit at that node's pressure)
+    gy[0, 1, 25] = 0.6
+    gy[0, 2, 25] = 1.3
+    gx[0, 3, 25] = 0.8
+    gy[0, 3, 26] = 1.7
+    gx[0, 4, 25] = 0.5
+    gy[0, 3, 25] = 1.2
+    net = type("N", (), dict(nx=nx, ny=ny, nz=1, gx=gx, gy=gy, gz=None, n_nodes=nx * ny, name="ladder"))()
+    for peel in (0, 1):
+        info, *_ = compare(pn, oracle, net, 0, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3, pn.PN_OPT_PEEL: peel})
+        assert info.kernel_scheme == 7 and info.n_chain > 40
