@@ -79,6 +79,8 @@ typedef struct {
     long long n_unknowns;  /* unknowns of the inner linear system: n_solved - n_peeled - n_chain           */
     long long n_chain;     /* solved nodes eliminated as links of degree-2 chains (PN_OPT_CONTRACT) and back-filled
                               by interpolation between the ends of their chain; counted in n_solved too   */
+    long long n_long_rows; /* compacted unknowns (kernel_scheme 7): rows of the neighbour table with more than three
+                              entries (they carry a 32-byte overflow record)                               */
     int labels_reused;     /* 1: S1's labelling and peeling were skipped, the classes of the previous solve
                               still hold (pn_update_conductances / pn_replace_conductances, no bond crossed zero) */
 } pn_info;

@@ -630,6 +630,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         info->labels_reused = reuse ? 1 : 0;
         info->n_unknowns = cm ? cm : n_solved - n_peeled;
         info->n_chain = (long long)h->n_chain;
+        info->n_long_rows = clong;
         if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) info->t_label_ms = ms;
         if (cudaEventElapsedTime(&ms, ctx->ev[1], ctx->ev[2]) == cudaSuccess) info->t_solve_ms = ms;
         info->t_stencil_ms = t_stencil;

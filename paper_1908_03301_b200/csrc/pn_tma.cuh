@@ -47,50 +47,10 @@ __device__ __forceinline__ void tma_load_3d(float* dst, const CUtensorMap* map, 
         "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
         : "memory");
 }
-// TMA load with an L2 eviction-priority hint (createpolicy): weights are read once per iteration and never reused
-// across CTAs (evict_first), the vectors' tile rows are re-read as halo rows by the neighbouring CTAs (evict_last)
-__device__ __forceinline__ uint64_t l2_policy_evict_first() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ void tma_load_3d_hint(float* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar,
-                                                 uint64_t policy) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(
-            smem_u32(dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)), "l"(policy)
-        : "memory");
-}
 // named barrier 1 over the first n threads of the CTA (the consumer warps)
 __device__ __forceinline__ void bar_consumers(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
 
 __device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-// Explicit ld.shared / st.shared for tile pointers whose address space the compiler cannot prove (a rounded-up dynamic
-// shared-memory base makes plain dereferences GENERIC accesses, LD.E / ST.E in SASS).  Which form is faster was measured
-// per kernel (profiles/r01_barrier_placement.md, profiles/r01_q_recompute_experiment.md).  `volatile`: never merged or
-// moved across the mbarrier waits and barriers.
-__device__ __forceinline__ float4 slds4(const float* p) {
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(smem_u32(p)));
-    return v;
-}
-__device__ __forceinline__ float slds1(const float* p) {
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(smem_u32(p)));
-    return v;
-}
-__device__ __forceinline__ void ssts4(float* p, const float4& v) {
-    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(p)), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
-}
-__device__ __forceinline__ void ssts1(float* p, float v) {
-    asm volatile("st.shared.f32 [%0], %1;" ::"r"(smem_u32(p)), "f"(v) : "memory");
-}
 __device__ __forceinline__ float4 fma4(float a, const float4& x, const float4& y) {
     return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
 }

@@ -43,7 +43,7 @@ class PnInfo(ctypes.Structure):
                 ("t_stencil_ms", ctypes.c_double), ("t_update_ms", ctypes.c_double),
                 ("n_timed_iters", ctypes.c_int), ("n_xskip", ctypes.c_int),
                 ("n_peeled", ctypes.c_longlong), ("n_unknowns", ctypes.c_longlong),
-                ("n_chain", ctypes.c_longlong), ("labels_reused", ctypes.c_int)]
+                ("n_chain", ctypes.c_longlong), ("n_long_rows", ctypes.c_longlong), ("labels_reused", ctypes.c_int)]
 
 
 @dataclass
@@ -68,6 +68,7 @@ class SolveInfo:
     labels_reused: int = 0
     n_unknowns: int = 0
     n_chain: int = 0
+    n_long_rows: int = 0
 
 
 class PnError(RuntimeError):
@@ -241,7 +242,7 @@ class Network:
         return SolveInfo(rc, info.outer_cycles, info.inner_iters, info.rel_residual, info.b_norm, info.n_solved,
                          info.n_inlet_only, info.n_outlet_only, info.n_floating, info.t_label_ms, info.t_solve_ms,
                          info.t_stencil_ms, info.t_update_ms, info.n_timed_iters, info.kernel_scheme, info.n_peeled, info.n_xskip,
-                         info.labels_reused, info.n_unknowns, info.n_chain)
+                         info.labels_reused, info.n_unknowns, info.n_chain, info.n_long_rows)
 
     def pressures(self, out=None):
         """fp64 pressures on all nodes as a CUDA tensor of shape (nz, ny, nx)."""
