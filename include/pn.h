@@ -125,7 +125,9 @@ enum {
                                first node (validated at pn_solve: PN_ERR_VALUE).  An axis of one node does
                                not wrap                                                             */
     PN_OPT_GRAPH = 9,       /* 1 (default): a chunk of inner iterations is replayed from a CUDA graph (captured
-                               once per geometry / direction / scheme); 0: every kernel launched directly  */
+                               once per geometry / direction / scheme); with the compacted unknowns (scheme 7): ONE
+                               persistent cooperative launch runs all iterations up to the next residual
+                               replacement.  0: every kernel launched directly, one by one                  */
     PN_OPT_REUSE_LABELS = 11, /* 1 (default): a solve that follows pn_update_conductances / pn_replace_conductances (or simply
                                repeats the previous one) keeps the node classes, pins and peeled set of the previous solve
                                when no bond went from closed to open or back and direction, PN_OPT_LATERAL, PN_OPT_PEEL

@@ -543,7 +543,10 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         // Graph path: whole chunks replayed from one executable graph.  With PN_OPT_PROFILE it is used for the single-kernel
         // scheme only (one kernel per iteration: the chunk's device time / iterations run is that kernel's average launch
         // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
-        const bool graph = ctx->use_graph && ctx->chunk > 1 && (scheme < 5 || scheme == 7) && !(ctx->profile && !fused) && ensure_graph(ctx, scheme, cm, clong);
+        // compacted unknowns: PN_OPT_GRAPH = 1 means the persistent cooperative launch (one per residual replacement);
+        // 0 the two kernels of an iteration launched one by one
+        const int lscheme = (scheme == 7 && ctx->use_graph && g.coop) ? 8 : scheme;
+        const bool graph = ctx->use_graph && ctx->chunk > 1 && lscheme < 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme, cm, clong);
         const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);   // (scheme 7: two kernels, never with wrap)
         while (true) {
             if (graph) {
@@ -552,7 +555,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 if (ctx->profile) CK(cudaEventRecord(ctx->pev[1], s));
                 nl += per_iter * ctx->chunk;
             } else {
-                CK(pn_launch_inner(g, P, ctx->chunk, scheme, s, &nl, ctx->profile ? ctx->pev : nullptr, &ctx->C));
+                CK(pn_launch_inner(g, P, ctx->chunk, lscheme, s, &nl, ctx->profile ? ctx->pev : nullptr, &ctx->C));
             }
             rc = read_state(ctx);
             if (rc) return rc;
@@ -561,7 +564,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
                 if (ran > 0) { t_stencil += ta; n_timed += ran; }
-            } else if (ctx->profile && (scheme == 5 || scheme == 6)) {   // one launch ran `ran` iterations (on chip / persistent)
+            } else if (ctx->profile && (lscheme == 5 || lscheme == 6 || lscheme == 8)) {   // one launch ran `ran` iterations (on chip / persistent)
                 const int ran = h->iters - iters_seen;
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);

@@ -328,6 +328,151 @@ __global__ void __launch_bounds__(TPB) k_cspmv(pn_ptrs P, pn_cptrs C) {
     }
 }
 
+// ---- the same iteration as ONE persistent cooperative launch per residual replacement ------------------------------------
+// With the links eliminated configs[2] has 1.7 M unknowns: the two kernels of an iteration take 21 us and their two
+// boundaries (launch gap, last-block reduction tail, start-up of 1184 CTAs) another 14 (profiles/r02_ncu.md).  Here every CTA
+// owns a fixed range of rows for the whole launch and the boundaries become two grid barriers per iteration: one after
+// the vector updates (the gathers read other CTAs' p_t), one after the operator (alpha, beta need the four sums).  As in
+// k_cg_resident2d, after the second barrier EVERY CTA adds the slots in the same fixed order and runs pn_finish_F on its
+// own copy of the state.  Same arithmetic per row as k_cupdate / k_cspmv; the partial sums are grouped per CTA range.
+constexpr int PT = 1024;
+
+__device__ __forceinline__ void cp_red_release_add(unsigned int* p, unsigned int v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned int cp_ld_relaxed(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// one thread per CTA, between two CTA barriers; __threadfence after the spin also drops the SM's L1 lines, so that the
+// plain loads that follow see what the other CTAs wrote
+__device__ __forceinline__ void cp_grid_barrier(unsigned int* bar, unsigned int target) {
+    cp_red_release_add(bar, 1u);
+    while (cp_ld_relaxed(bar) < target) { }
+    __threadfence();
+}
+
+// one table row (shared by the persistent kernel's operator phase)
+__device__ __forceinline__ float row_sum(const pn_cptrs& C, const float* __restrict__ p, int c0, int c1, int c2, float v0, float v1,
+                                         float v2) {
+    float acc = v0 * p[c0];
+    acc = fmaf(v1, p[c1], acc);
+    if (c2 >= 0) acc = fmaf(v2, p[c2], acc);
+    else {
+        const int4 oc = reinterpret_cast<const int4*>(C.ovc)[-1 - c2];
+        const float4 ov = reinterpret_cast<const float4*>(C.ovv)[-1 - c2];
+        acc = fmaf(ov.x, p[oc.x], acc);
+        acc = fmaf(ov.y, p[oc.y], acc);
+        acc = fmaf(ov.z, p[oc.z], acc);
+        acc = fmaf(ov.w, p[oc.w], acc);
+    }
+    return acc;
+}
+
+__global__ void __launch_bounds__(PT, 1) k_cpersist(pn_ptrs P, pn_cptrs C, int max_launch_iters) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;   // same value in every CTA: nobody enters the barriers alone
+    __shared__ double red[4 * 32 + 8];
+    __shared__ pn_state ls;                 // this CTA's copy of the iteration state
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int G = (int)gridDim.x, c = (int)blockIdx.x;
+    if (tid == 0) ls = *st;
+    __syncthreads();
+    const long long m = (long long)ls.cm;
+    const long long per = ((m + 4ll * G - 1) / (4ll * G)) * 4;             // rows per CTA, a multiple of 4
+    const long long i0 = min(per * c, m), i1 = min(i0 + per, m);
+    const long long v0i = i0 >> 2, v1i = i1 >> 2;                           // whole groups of 4 rows in [i0, i1)
+    const long long t0i = max(4 * v1i, i0);                                 // the range's last 0..3 rows (an empty range has none)
+    const float* __restrict__ p = C.p;
+    unsigned int* bar = P.gbar;
+    unsigned int bar_target = 0;
+
+    for (int li = 0; li < max_launch_iters; ++li) {
+        const int pin = li & 1;
+        const float al = (float)ls.alpha, nal = -al, beta = (float)ls.beta;
+        double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
+        // ---- r_t = r - alpha q ; x_hat += alpha p ; p_t = r_t + beta p ; r_t.r_t (own rows) ----
+        for (long long v = v0i + tid; v < v1i; v += PT) {
+            const long long i = 4 * v;
+            float4 r = ld4(C.r + i);
+            const float4 q = ld4(C.q + i);
+            float4 pp = ld4(C.p + i), x = ld4(C.x + i);
+            r.x = fmaf(nal, q.x, r.x); r.y = fmaf(nal, q.y, r.y); r.z = fmaf(nal, q.z, r.z); r.w = fmaf(nal, q.w, r.w);
+            x.x = fmaf(al, pp.x, x.x); x.y = fmaf(al, pp.y, x.y); x.z = fmaf(al, pp.z, x.z); x.w = fmaf(al, pp.w, x.w);
+            pp.x = fmaf(beta, pp.x, r.x); pp.y = fmaf(beta, pp.y, r.y); pp.z = fmaf(beta, pp.z, r.z); pp.w = fmaf(beta, pp.w, r.w);
+            st4(C.r + i, r); st4(C.x + i, x); st4(C.p + i, pp);
+            a_rr += (double)(r.x * r.x + r.y * r.y + r.z * r.z + r.w * r.w);
+        }
+        for (long long i = t0i + tid; i < i1; i += PT) {
+            const float r = fmaf(nal, C.q[i], C.r[i]);
+            const float pp = C.p[i];
+            C.x[i] = fmaf(al, pp, C.x[i]);
+            C.r[i] = r;
+            C.p[i] = fmaf(beta, pp, r);
+            a_rr += (double)(r * r);
+        }
+        __syncthreads();
+        if (tid == 0) { bar_target += G; cp_grid_barrier(bar, bar_target); }
+        __syncthreads();
+        // ---- q_t = p_t - W p_t over the table rows (own rows; the gathers reach any row) ; p.q, r.q, q.q ----
+        for (long long v = v0i + tid; v < v1i; v += PT) {
+            const long long i = 4 * v;
+            const int4 c0 = *reinterpret_cast<const int4*>(C.c[0] + i), c1 = *reinterpret_cast<const int4*>(C.c[1] + i),
+                       c2 = *reinterpret_cast<const int4*>(C.c[2] + i);
+            const float4 w0 = ld4(C.v[0] + i), w1 = ld4(C.v[1] + i), w2 = ld4(C.v[2] + i);
+            const float4 pi = ld4(p + i), ri = ld4(C.r + i);
+            float4 q;
+            q.x = pi.x - row_sum(C, p, c0.x, c1.x, c2.x, w0.x, w1.x, w2.x);
+            q.y = pi.y - row_sum(C, p, c0.y, c1.y, c2.y, w0.y, w1.y, w2.y);
+            q.z = pi.z - row_sum(C, p, c0.z, c1.z, c2.z, w0.z, w1.z, w2.z);
+            q.w = pi.w - row_sum(C, p, c0.w, c1.w, c2.w, w0.w, w1.w, w2.w);
+            st4(C.q + i, q);
+            a_pq += (double)(pi.x * q.x + pi.y * q.y + pi.z * q.z + pi.w * q.w);
+            a_rq += (double)(ri.x * q.x + ri.y * q.y + ri.z * q.z + ri.w * q.w);
+            a_qq += (double)(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
+        }
+        for (long long i = t0i + tid; i < i1; i += PT) {
+            const float pi = p[i];
+            const float q = pi - row_sum(C, p, C.c[0][i], C.c[1][i], C.c[2][i], C.v[0][i], C.v[1][i], C.v[2][i]);
+            C.q[i] = q;
+            a_pq += (double)(pi * q);
+            a_rq += (double)(C.r[i] * q);
+            a_qq += (double)(q * q);
+        }
+        // ---- the four sums: warp -> CTA -> slots -> grid barrier -> every CTA adds the slots in the same order ----
+        a_rr = pn_warp_sum(a_rr); a_pq = pn_warp_sum(a_pq); a_rq = pn_warp_sum(a_rq); a_qq = pn_warp_sum(a_qq);
+        if (lane == 0) { red[wid] = a_rr; red[32 + wid] = a_pq; red[64 + wid] = a_rq; red[96 + wid] = a_qq; }
+        __syncthreads();
+        if (wid == 0) {
+            double* my = P.slots + ((size_t)pin * PN_MAX_BLOCKS + c) * 4;     // [parity][CTA][4]: one 32-byte sector per CTA
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double v = pn_warp_sum(red[32 * k + lane]);
+                if (lane == 0) my[k] = v;
+            }
+            if (lane == 0) { bar_target += G; cp_grid_barrier(bar, bar_target); }
+            __syncwarp();
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+            const double2* sl = reinterpret_cast<const double2*>(P.slots + (size_t)pin * PN_MAX_BLOCKS * 4);
+            double2 va[(PN_RESIDENT_MAX_CTAS + 31) / 32], vb[(PN_RESIDENT_MAX_CTAS + 31) / 32];
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) {
+                const int b = lane + 32 * u;
+                va[u] = b < G ? __ldcg(sl + 2 * b) : make_double2(0.0, 0.0);
+                vb[u] = b < G ? __ldcg(sl + 2 * b + 1) : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) { t0 += va[u].x; t1 += va[u].y; t2 += vb[u].x; t3 += vb[u].y; }
+            t0 = pn_warp_sum(t0); t1 = pn_warp_sum(t1); t2 = pn_warp_sum(t2); t3 = pn_warp_sum(t3);
+            if (lane == 0) pn_finish_F(&ls, t0, t1, t2, t3);
+        }
+        __syncthreads();
+        if (ls.flag != PN_FLAG_RUN) break;
+    }
+    if (c == 0 && tid == 0) *st = ls;
+}
+
 }  // namespace
 
 // Where the compact arrays live: in lattice-shaped arrays the structured kernels do not need during a compact solve.
@@ -401,6 +546,17 @@ cudaError_t pn_launch_compact_flush(const pn_geom& g, const pn_ptrs& P, const pn
     k_cflush<<<grid_for(m, g.sms), TPB, 0, st>>>(P, C);
     ++*launches;
     return cudaGetLastError();
+}
+
+// All iterations up to the next trigger in ONE cooperative launch (k_cpersist)
+cudaError_t pn_launch_compact_persist(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, int max_launch_iters, cudaStream_t st) {
+    int G = g.sms < PN_RESIDENT_MAX_CTAS ? g.sms : PN_RESIDENT_MAX_CTAS;
+    cudaError_t e = cudaMemsetAsync(P.gbar, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+    pn_ptrs PP = P;
+    pn_cptrs CC = C;
+    void* args[] = {(void*)&PP, (void*)&CC, (void*)&max_launch_iters};
+    return cudaLaunchCooperativeKernel((const void*)k_cpersist, dim3(G), dim3(PT), args, 0, st);
 }
 
 // `iterations` iterations of the compact scheme: two launches each

@@ -181,7 +181,15 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
         *launches += 1;
         return e5;
     }
-    if (scheme == 7) return compact ? pn_launch_compact_inner(g, P, *compact, iterations, st, launches, ev) : cudaErrorInvalidValue;   // compacted unknowns (pn_compact.cu)
+    if (scheme == 7 || scheme == 8) {   // compacted unknowns (pn_compact.cu): two kernels per iteration / one persistent launch
+        if (!compact) return cudaErrorInvalidValue;
+        if (scheme == 7) return pn_launch_compact_inner(g, P, *compact, iterations, st, launches, ev);
+        if (ev) cudaEventRecord(ev[0], st);
+        cudaError_t e8 = pn_launch_compact_persist(g, P, *compact, 1 << 30, st);
+        if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
+        *launches += 1;
+        return e8;
+    }
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];   // periodic lateral faces: k_wrap_fix finishes kernel A
     cudaError_t e = cudaSuccess;
     if (ev) cudaEventRecord(ev[0], st);

@@ -288,6 +288,7 @@ cudaError_t pn_launch_compact_flush(const pn_geom& g, const pn_ptrs& P, const pn
                                     int* launches);
 cudaError_t pn_launch_compact_inner(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, int iterations, cudaStream_t st,
                                     int* launches, cudaEvent_t* ev);
+cudaError_t pn_launch_compact_persist(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, int max_launch_iters, cudaStream_t st);
 
 // Persistent in-place iteration for 2D lattices (pn_resident.cu): all iterations up to the next trigger in ONE cooperative launch
 bool pn_resident_supported(const pn_geom& g, const pn_ptrs& P);
