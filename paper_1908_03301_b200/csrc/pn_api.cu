@@ -479,7 +479,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         const long long m = (long long)ctx->h_state->cm, nl_rows = (long long)ctx->h_state->clong;
         const bool want = ctx->compact == 1 || (double)m <= PN_COMPACT_MAX_FRACTION * (double)g.npad;
         if (want && pn_compact_fits(g, m, nl_rows)) {
-            ctx->C = pn_compact_ptrs(P, m, nl_rows);
+            ctx->C = pn_compact_ptrs(g, P, m, nl_rows);
             CK(pn_launch_compact_build(g, P, ctx->C, m, chains, s, &nl));
             cm = m; clong = nl_rows;
             scheme = 7; fused = 1; bufmode = 2;
@@ -495,7 +495,17 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     ctx->warm_next = false;
     ctx->label_dir = g.dir; ctx->label_lateral = ctx->lateral; ctx->label_peel = ctx->peel; ctx->label_skip = ctx->skip_label;
     ctx->label_chains = chains; ctx->label_compact = ctx->compact; ctx->label_contract = ctx->contract; ctx->label_variant = ctx->variant;
-    if (chains) CK(pn_launch_chain_fill(g, P, s, &nl));   // chain nodes follow the starting pressures of their chains' ends
+    // back-fill of the chain nodes: by one record per node written once per solve when the records fit the arrays the
+    // compact form leaves free (else by walking the chains every time)
+    long long n_rec = 0;
+    if (chains && cm && (long long)ctx->h_state->n_chain <= ctx->C.chcap) {
+        n_rec = (long long)ctx->h_state->n_chain;
+        CK(pn_launch_chain_record(g, P, ctx->C, s, &nl));
+    }
+    auto chain_fill = [&]() -> cudaError_t {
+        return n_rec ? pn_launch_chain_fill_rec(g, P, ctx->C, n_rec, s, &nl) : pn_launch_chain_fill(g, P, s, &nl);
+    };
+    if (chains) CK(chain_fill());   // chain nodes follow the starting pressures of their chains' ends
     CK(pn_launch_residual64(g, P, bufmode, s, &nl));
     if (cm) CK(pn_launch_compact_gather(g, P, ctx->C, cm, s, &nl));
     CK(cudaEventRecord(ctx->ev[1], s));
@@ -589,7 +599,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
             const int flag = h->flag;
             if (cm) CK(pn_launch_compact_flush(g, P, ctx->C, cm, s, &nl));
             else CK(pn_launch_flush(g, P, bufmode, s, &nl));
-            if (chains) CK(pn_launch_chain_fill(g, P, s, &nl));
+            if (chains) CK(chain_fill());
             CK(pn_launch_residual64(g, P, bufmode, s, &nl));
             if (cm) CK(pn_launch_compact_gather(g, P, ctx->C, cm, s, &nl));
             rc = read_state(ctx);

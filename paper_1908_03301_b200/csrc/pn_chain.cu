@@ -105,7 +105,70 @@ __global__ void k_chain_fill(pn_geom g, pn_ptrs P) {
     }
 }
 
+// The same walk, once per solve: instead of pressures it leaves one record per chain node -- (node, a, b, t) with
+// t = R(a -> node) / R(a -> b) -- so that every later back-fill is a flat gather (k_chain_fill_rec) instead of 3.9 M
+// dependent-load walks (configs[2]: 1.8 ms per walk-based fill, ~20 of them per solve, against 0.05 ms).  Record slots
+// are handed out by an atomic counter: their order varies from run to run, what each holds does not.
+__global__ void k_chain_record(pn_geom g, pn_ptrs P, pn_cptrs C) {
+    for (long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x; a < g.npad; a += (long long)gridDim.x * blockDim.x) {
+        if (P.cls[a] != PN_CLASS_SOLVED) continue;
+#pragma unroll 1
+        for (int dir = 0; dir < 6; ++dir) {
+            long long first;
+            const float g0 = pn_bond_dir(g, P, a, dir, &first);
+            if (g0 == 0.f || P.cls[first] != PN_CLASS_CHAIN) continue;
+            const pn_walk w = pn_walk_chain(g, P, a, dir);
+            if (w.end < a || (w.end == a && w.last < first)) continue;   // the other end (or the other way round the loop) does it
+            const double inv = w.end == a ? 0.0 : 1.0 / w.R;
+            long long prev = a, cur = first;
+            double R = 1.0 / (double)g0;
+            while (P.cls[cur] == PN_CLASS_CHAIN) {
+                const unsigned long long slot = atomicAdd(&P.st->n_rec, 1ull);
+                if ((long long)slot < C.chcap) {
+                    C.chv[slot] = (int)cur;
+                    C.chab[slot] = make_int2((int)a, (int)w.end);
+                    C.cht[slot] = R * inv;
+                }
+                long long nxt = -1;
+                float gn = 0.f;
+#pragma unroll
+                for (int d = 0; d < 6; ++d) {
+                    long long m;
+                    const float gv = pn_bond_dir(g, P, cur, d, &m);
+                    if (gv != 0.f && m != prev) { nxt = m; gn = gv; }
+                }
+                if (nxt < 0) break;
+                R += 1.0 / (double)gn;
+                prev = cur;
+                cur = nxt;
+            }
+        }
+    }
+}
+
+__global__ void k_chain_fill_rec(pn_ptrs P, pn_cptrs C, long long n) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        const int2 ab = C.chab[j];
+        const double xa = P.x64[ab.x];
+        P.x64[C.chv[j]] = xa + C.cht[j] * (P.x64[ab.y] - xa);
+    }
+}
+
 }  // namespace
+
+cudaError_t pn_launch_chain_record(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, cudaStream_t st, int* launches) {
+    cudaError_t e = cudaMemsetAsync(&P.st->n_rec, 0, sizeof(P.st->n_rec), st);
+    if (e != cudaSuccess) return e;
+    k_chain_record<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P, C);
+    ++*launches;
+    return cudaGetLastError();
+}
+cudaError_t pn_launch_chain_fill_rec(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long n_chain, cudaStream_t st,
+                                     int* launches) {
+    k_chain_fill_rec<<<grid_for(n_chain, g.sms), TPB, 0, st>>>(P, C, n_chain);
+    ++*launches;
+    return cudaGetLastError();
+}
 
 cudaError_t pn_launch_chain_mark(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches) {
     k_chain_mark<<<grid_for(g.npad, g.sms), TPB, 0, st>>>(g, P);

@@ -21,6 +21,9 @@
 // adjacent and y / z neighbours a fixed few thousand entries away: the gathers are served by L1 / L2.
 // The fp64 outer steps stay on the lattice (k_residual64 writes r_hat there); k_cgather / k_cflush move r_hat and the
 // correction between the two numberings.  No periodic faces (those lattices keep the structured kernels).
+// With PN_OPT_CONTRACT the degree-2 link nodes are eliminated first (pn_chain.cu): a bond towards a chain becomes a table
+// entry to the chain's far end.  By default the two kernels run as the two phases of ONE persistent cooperative launch
+// per residual replacement (k_cpersist, below); kernel by kernel with PN_OPT_GRAPH = 0.
 #include "pn_chain.cuh"
 
 namespace {
@@ -485,7 +488,7 @@ bool pn_compact_fits(const pn_geom& g, long long m, long long n_long) {
     return m >= 1 && 2 * off <= g.npad && off + 8 * n_long + 8 <= g.npad;
 }
 
-pn_cptrs pn_compact_ptrs(const pn_ptrs& P, long long m, long long n_long) {
+pn_cptrs pn_compact_ptrs(const pn_geom& g, const pn_ptrs& P, long long m, long long n_long) {
     const long long off = (m + 63) & ~63ll;
     pn_cptrs C;
     C.cidx = (int*)P.r;
@@ -499,6 +502,16 @@ pn_cptrs pn_compact_ptrs(const pn_ptrs& P, long long m, long long n_long) {
     C.x = P.xh;
     C.q = P.w[0];
     C.r = P.w[1];
+    // back-fill records of the chain nodes: the node list in the unused upper half of w[0]; (a, b) and t in the upper half
+    // of w[1] and all of w[2] (consecutive in the workspace; the weights are dead once the table is built)
+    C.chv = (int*)P.w[0] + off;
+    char* lo = (char*)(P.w[1] + off);
+    long long cap = (long long)((char*)(P.w[2] + g.npad) - lo) / 16;
+    if (cap > g.npad - off) cap = g.npad - off;
+    if (cap < 0) cap = 0;
+    C.chab = reinterpret_cast<int2*>(lo);
+    C.cht = reinterpret_cast<double*>(lo + 8 * cap);
+    C.chcap = cap;
     return C;
 }
 

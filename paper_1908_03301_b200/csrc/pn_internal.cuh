@@ -72,6 +72,7 @@ struct pn_state {
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
     unsigned long long n_peeled;// solved nodes removed from the system as dangling ends (back-filled after the solve)
     unsigned long long n_chain; // solved nodes eliminated as links of degree-2 chains (pn_chain.cu; back-filled)
+    unsigned long long n_rec;   // back-fill records written so far (k_chain_record)
     unsigned long long cm;      // active-node compaction (pn_compact.cu): unknowns of the inner system ...
     unsigned long long clong;   // ... and rows of its neighbour table with more than three entries
     int flag;                   // 0 run, 1 proxy-converged, 2 reliable update due, 3 breakdown, 4 budget
@@ -265,6 +266,10 @@ cudaError_t pn_launch_chain_mark(const pn_geom& g, const pn_ptrs& P, cudaStream_
 cudaError_t pn_launch_chain_unmark(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_chain_scale(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
 cudaError_t pn_launch_chain_fill(const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int* launches);
+struct pn_cptrs;
+cudaError_t pn_launch_chain_record(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, cudaStream_t st, int* launches);
+cudaError_t pn_launch_chain_fill_rec(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long n_chain, cudaStream_t st,
+                                     int* launches);
 
 // Active-node compaction (pn_compact.cu): the inner iteration on the unknowns only, ELL-3 + overflow neighbour table
 struct pn_cptrs {
@@ -275,9 +280,15 @@ struct pn_cptrs {
     int* ovc;                   // overflow records: entries 3..6 of the long rows, 4 indices ...
     float* ovv;                 // ... and 4 weights per record
     float *r, *q, *p, *x;       // cm entries each
+    // degree-2 chains (pn_chain.cu): one back-fill record per chain node, written once per solve -- the node, the two ends
+    // of its chain (lattice indices) and its share t of the chain's resistance: P_node = P_a + t (P_b - P_a)
+    int* chv;
+    int2* chab;
+    double* cht;
+    long long chcap;            // records these arrays hold (0: none -- the back-fill walks the chains every time)
 };
 bool pn_compact_fits(const pn_geom& g, long long m, long long n_long);
-pn_cptrs pn_compact_ptrs(const pn_ptrs& P, long long m, long long n_long);
+pn_cptrs pn_compact_ptrs(const pn_geom& g, const pn_ptrs& P, long long m, long long n_long);
 // `chains`: degree-2 chain nodes are marked (pn_chain.cu): a bond towards one is a table entry to the chain's far end
 cudaError_t pn_launch_compact_count(const pn_geom& g, const pn_ptrs& P, int chains, cudaStream_t st, int* launches);
 cudaError_t pn_launch_compact_build(const pn_geom& g, const pn_ptrs& P, const pn_cptrs& C, long long m, int chains,
