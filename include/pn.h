@@ -62,7 +62,7 @@ typedef struct {
     int status;            /* the code pn_solve returned                                            */
     int outer_cycles;      /* fp64 true-residual evaluations  r = b - A x  (S8(a) S3)                */
     int inner_iters;       /* fp32 CG iterations (S8(a) S4+S5), summed over the solve               */
-    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3, 5 or 6), or 7 = compacted unknowns (PN_OPT_COMPACT) */
+    int kernel_scheme;     /* inner-iteration kernels used: the resolved PN_OPT_KERNEL value (1, 3, 5, 6 or 8), or 7 = compacted unknowns (PN_OPT_COMPACT) */
     double rel_residual;   /* true fp64 ||b - A x||_2 / ||b||_2 over the solved nodes at exit       */
     double b_norm;         /* ||b||_2 of the zero-initial-guess system (S8(c) reading 5)            */
     long long n_solved, n_inlet_only, n_outlet_only, n_floating; /* interior node counts by class    */
@@ -100,14 +100,17 @@ enum {
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
                                memory -- at most 7168 padded floats per array, no periodic faces --, 6 where it
-                               applies, 1 on other lattices of at most 600 000 padded nodes, else 3),
+                               applies, 8 on other lattices of at most 5 000 000 padded nodes, else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept as an independently written cross-check),
                                3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
                                5 = the whole inner loop in ONE launch of one CTA, vectors in shared memory,
                                6 = 2D lattices whose rows / SMs slabs fit the SMs' shared memory (about 1.2 M nodes,
                                at most 2048 wide, no periodic faces): ONE persistent cooperative launch per residual
-                               replacement, every CTA keeping its slab on chip, grid barrier per iteration; else 3.
+                               replacement, every CTA keeping its slab on chip, grid barrier per iteration; else 3,
+                               8 = any lattice without periodic faces: ONE persistent cooperative launch per residual
+                               replacement, vectors in HBM / L2, two grid barriers per iteration (for lattices that
+                               sit in the L2, where an iteration is bound by launches, not by HBM); with periodic faces: 1.
                                (2 and 4 were round-1 experiments, since removed: PN_ERR_ARG)                   */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */

@@ -250,7 +250,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_X0: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
         case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
-        case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0 && value != 6.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
+        case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0 && value != 6.0 && value != 8.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
@@ -408,8 +408,8 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     CK(cudaMemsetAsync(&P.st->ticket, 0, sizeof(unsigned int), s));
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     int scheme = pn_resolve_variant(g, P, ctx->variant);
-    int fused = scheme == 3 || scheme == 6;   // deferred residual update + predicted beta (the state holds the measured r.r)
-    int bufmode = scheme == 3 ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
+    int fused = scheme == 3 || scheme == 6 || scheme == 8;   // deferred residual update + predicted beta (the state holds the measured r.r)
+    int bufmode = scheme == 3 ? 1 : ((scheme == 6 || scheme == 8) ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -442,7 +442,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     }
     // active-node compaction may apply (decided below, once the scaled weights exist): automatic only with the automatic
     // kernel choice -- an explicit PN_OPT_KERNEL is honoured unless PN_OPT_COMPACT = 1
-    const bool compact_allowed = (ctx->compact == 1 || (ctx->compact == 2 && ctx->variant == 0)) && !any_wrap && (scheme == 3 || scheme == 1);
+    const bool compact_allowed = (ctx->compact == 1 || (ctx->compact == 2 && ctx->variant == 0)) && !any_wrap && (scheme == 3 || scheme == 1 || scheme == 8);
     // degree-2 chain nodes (pn_chain.cu) are eliminated together with the compaction: marked now, because the Jacobi scale
     // and the weights of the reduced system depend on them
     int chains = 0;
@@ -539,7 +539,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         rn = 0.0;
     } else if (rn > tol * nb) {
         const double delta2 = ctx->delta * ctx->delta;
-        const double xskip_min = (fused && scheme != 7 && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
+        const double xskip_min = (fused && scheme != 7 && scheme != 8 && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
         auto target_for = [&](double rn_true, double rr_true) {
             // proxy of the fp64 exit test in the scaled norm: ||r|| / ||r_hat|| measured at this replacement
             const double c = rn_true / sqrt(rr_true);
@@ -555,7 +555,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
         // compacted unknowns: PN_OPT_GRAPH = 1 means the persistent cooperative launch (one per residual replacement);
         // 0 the two kernels of an iteration launched one by one
-        const int lscheme = (scheme == 7 && ctx->use_graph && g.coop) ? 8 : scheme;
+        const int lscheme = (scheme == 7 && ctx->use_graph && g.coop) ? 9 : scheme;
         const bool graph = ctx->use_graph && ctx->chunk > 1 && lscheme < 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme, cm, clong);
         const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);   // (scheme 7: two kernels, never with wrap)
         while (true) {
@@ -574,7 +574,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
                 if (ran > 0) { t_stencil += ta; n_timed += ran; }
-            } else if (ctx->profile && (lscheme == 5 || lscheme == 6 || lscheme == 8)) {   // one launch ran `ran` iterations (on chip / persistent)
+            } else if (ctx->profile && (lscheme == 5 || lscheme == 6 || lscheme == 8 || lscheme == 9)) {   // one launch ran `ran` iterations (on chip / persistent)
                 const int ran = h->iters - iters_seen;
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);

@@ -133,6 +133,115 @@ __global__ void __launch_bounds__(TPB) k_update(int nvec, pn_ptrs P) {
     }
 }
 
+// ---- the same iteration for SMALL lattices as ONE persistent cooperative launch per residual replacement -----------------
+// Below ~600 000 nodes an iteration is bound by launches, not by memory (12.5 us at 64^3 for the pair above, of which the
+// two kernels' work is a fraction; profiles/r02_small_lattices.md).  Here every CTA owns a fixed range of the lattice for the
+// whole launch; an iteration is two phases with the recurrences of the single-kernel scheme (deferred residual update,
+// predicted beta: pn_finish_F) separated by two grid barriers:
+//   phase U   r_t = r - alpha q ;  x_hat += alpha p ;  p_t = r_t + beta p ;  r_t.r_t              (own nodes)
+//   barrier   (the stencil reads other CTAs' p_t)
+//   phase S   q_t = p_t - W p_t, neighbours through L1 / L2 as in k_stencil_simple ;  p.q, r.q, q.q   (own nodes)
+//   barrier + every CTA adds the slots in the same fixed order and runs pn_finish_F on its own copy of the state
+// (k_cg_resident2d and k_cpersist work the same way).  Vectors live in one buffer each (P.r, P.q, P.p).
+constexpr int ST = 1024;
+
+__device__ __forceinline__ void sp_grid_barrier(unsigned int* bar, unsigned int target) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
+    unsigned int v;
+    do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory"); } while (v < target);
+    __threadfence();   // acquire; also drops the SM's L1 lines, so that the plain loads that follow see the other CTAs' stores
+}
+
+__global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int max_launch_iters) {
+    pn_state* st = P.st;
+    if (st->flag != PN_FLAG_RUN) return;   // same value in every CTA: nobody enters the barriers alone
+    __shared__ double red[4 * 32 + 8];
+    __shared__ pn_state ls;                 // this CTA's copy of the iteration state
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int G = (int)gridDim.x, c = (int)blockIdx.x;
+    if (tid == 0) ls = *st;
+    __syncthreads();
+    const long long nvec = g.npad >> 2;
+    const long long per = (nvec + G - 1) / G;
+    const long long v0 = min(per * c, nvec), v1 = min(v0 + per, nvec);
+    const int px = g.px;
+    const long long plane = g.plane;
+    const float* __restrict__ wx = P.w[0];
+    const float* __restrict__ wy = P.w[1];
+    const float* __restrict__ wz = P.w[2];
+    float* __restrict__ r = P.r;
+    float* __restrict__ q = P.q;
+    float* __restrict__ p = P.p;
+    unsigned int* bar = P.gbar;
+    unsigned int bar_target = 0;
+
+    for (int li = 0; li < max_launch_iters; ++li) {
+        const int pin = li & 1;
+        const float al = (float)ls.alpha, nal = -al, beta = (float)ls.beta;
+        double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
+        for (long long v = v0 + tid; v < v1; v += ST) {
+            const long long n = 4 * v;
+            const float4 qq = ld4(q + n), po = ld4(p + n);
+            const float4 rn = fma4(nal, qq, ld4(r + n));
+            st4(P.xh + n, fma4(al, po, ld4(P.xh + n)));
+            st4(r + n, rn);
+            st4(p + n, fma4(beta, po, rn));
+            a_rr += (double)(rn.x * rn.x + rn.y * rn.y + rn.z * rn.z + rn.w * rn.w);
+        }
+        __syncthreads();
+        if (tid == 0) { bar_target += G; sp_grid_barrier(bar, bar_target); }
+        __syncthreads();
+        for (long long v = v0 + tid; v < v1; v += ST) {
+            const long long n = 4 * v;
+            const float4 pn = ld4(p + n);
+            const float pl = p[n - 1], pr = p[n + 4];
+            const float4 pym = ld4(p + n - px), pyp = ld4(p + n + px), pzm = ld4(p + n - plane), pzp = ld4(p + n + plane);
+            const float4 gx = ld4(wx + n), gy = ld4(wy + n), gz = ld4(wz + n);
+            const float gxl = wx[n - 1];
+            const float4 gym = ld4(wy + n - px), gzm = ld4(wz + n - plane);
+            float4 qv;
+            qv.x = pn.x - (gxl * pl + gx.x * pn.y + gym.x * pym.x + gy.x * pyp.x + gzm.x * pzm.x + gz.x * pzp.x);
+            qv.y = pn.y - (gx.x * pn.x + gx.y * pn.z + gym.y * pym.y + gy.y * pyp.y + gzm.y * pzm.y + gz.y * pzp.y);
+            qv.z = pn.z - (gx.y * pn.y + gx.z * pn.w + gym.z * pym.z + gy.z * pyp.z + gzm.z * pzm.z + gz.z * pzp.z);
+            qv.w = pn.w - (gx.z * pn.z + gx.w * pr + gym.w * pym.w + gy.w * pyp.w + gzm.w * pzm.w + gz.w * pzp.w);
+            st4(q + n, qv);
+            const float4 rn = ld4(r + n);
+            a_pq += (double)(pn.x * qv.x + pn.y * qv.y + pn.z * qv.z + pn.w * qv.w);
+            a_rq += (double)(rn.x * qv.x + rn.y * qv.y + rn.z * qv.z + rn.w * qv.w);
+            a_qq += (double)(qv.x * qv.x + qv.y * qv.y + qv.z * qv.z + qv.w * qv.w);
+        }
+        a_rr = pn_warp_sum(a_rr); a_pq = pn_warp_sum(a_pq); a_rq = pn_warp_sum(a_rq); a_qq = pn_warp_sum(a_qq);
+        if (lane == 0) { red[wid] = a_rr; red[32 + wid] = a_pq; red[64 + wid] = a_rq; red[96 + wid] = a_qq; }
+        __syncthreads();
+        if (wid == 0) {
+            double* my = P.slots + ((size_t)pin * PN_MAX_BLOCKS + c) * 4;     // [parity][CTA][4]: one 32-byte sector per CTA
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double v = pn_warp_sum(red[32 * k + lane]);
+                if (lane == 0) my[k] = v;
+            }
+            if (lane == 0) { bar_target += G; sp_grid_barrier(bar, bar_target); }
+            __syncwarp();
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+            const double2* sl = reinterpret_cast<const double2*>(P.slots + (size_t)pin * PN_MAX_BLOCKS * 4);
+            double2 va[(PN_RESIDENT_MAX_CTAS + 31) / 32], vb[(PN_RESIDENT_MAX_CTAS + 31) / 32];
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) {
+                const int b = lane + 32 * u;
+                va[u] = b < G ? __ldcg(sl + 2 * b) : make_double2(0.0, 0.0);
+                vb[u] = b < G ? __ldcg(sl + 2 * b + 1) : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) { t0 += va[u].x; t1 += va[u].y; t2 += vb[u].x; t3 += vb[u].y; }
+            t0 = pn_warp_sum(t0); t1 = pn_warp_sum(t1); t2 = pn_warp_sum(t2); t3 = pn_warp_sum(t3);
+            if (lane == 0) pn_finish_F(&ls, t0, t1, t2, t3);
+        }
+        __syncthreads();
+        if (ls.flag != PN_FLAG_RUN) break;
+    }
+    if (c == 0 && tid == 0) *st = ls;
+}
+
 int grid_for(long long work_items, int sms) {
     long long nb = (work_items + TPB - 1) / TPB;
     long long cap = (long long)sms * 8;
@@ -145,22 +254,26 @@ int grid_for(long long work_items, int sms) {
 }  // namespace
 
 // PN_OPT_KERNEL: 0 = automatic: the whole loop in one CTA when the lattice fits one SM's shared memory (5); the persistent
-// shared-memory-resident kernel for 2D lattices whose slabs fit all SMs (6); the cache-fed pair below (1) for the other
-// lattices of at most PN_SMALL_LATTICE padded nodes; else the single fused TMA kernel (3).  Measured on B200 with BOTH
-// schemes replayed from CUDA graphs (profiles/r02_small_lattices.md; round 1's table had timed the pair without graph
-// replay): per iteration, pair / fused = 12.5 / 15.6 us at 64^3, 19.6 / 19.4 at 96^3, 26.1 / 26.1 at 128^3 -- the fused
-// kernel pays ~16 us of TMA ring ramp and reduction tail per launch, which only lattices from ~1 M nodes up amortise.
+// shared-memory-resident kernel for 2D lattices whose slabs fit all SMs (6); the persistent structured kernel above (8)
+// for the other lattices of at most PN_SMALL_LATTICE padded nodes (with periodic faces: the cache-fed pair, 1); else the
+// single fused TMA kernel (3).  Measured on B200 (profiles/r02_small_lattices.md), per iteration, persistent / pair /
+// fused: 7.8 / 12.2 / 15.3 us at 64^3, 10.7 / 19.3 / 19.1 at 96^3, 16.7 / - / 26.0 at 128^3, 33.9 / - / 43.1 at 160^3,
+// 69.6 / - / 61.0 at 192^3, 180 / - / 120 at 256^3; 2D: 14.9 / - / 27.1 at 1448^2, 34.0 / - / 34.3 at 2048^2.  The fused
+// kernel pays ~16 us of TMA ring ramp and reduction tail per launch but moves 40 instead of 52 bytes per node: it wins
+// once the lattice no longer sits in the L2 (from ~5 M nodes).
 // 1 = the pair on any lattice (independently written cross-check).  The two superseded schemes of round 1 (2: TMA S4
 // kernel + S5 kernel, 4: q recomputed) are gone; their write-ups remain in profiles/r01_tma_kernel.md and
-// profiles/r01_q_recompute_experiment.md.  6 = persistent in-place kernel for 2D lattices (pn_resident.cu).
-constexpr long long PN_SMALL_LATTICE = 600000;
+// profiles/r01_q_recompute_experiment.md.
+constexpr long long PN_SMALL_LATTICE = 5000000;
 int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant) {
     const int big = pn_tma_supported() ? 3 : 1;
     if (variant == 0) {
         if (pn_onchip_supported(g)) return 5;
         if (pn_resident_supported(g, P)) return 6;
-        return g.npad <= PN_SMALL_LATTICE ? 1 : big;
+        if (g.npad <= PN_SMALL_LATTICE) return (g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2])) ? 8 : 1;
+        return big;
     }
+    if (variant == 8 && !(g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2]))) return 1;   // periodic faces / no cooperative launch
     if (variant == 5 && !pn_onchip_supported(g)) return big;   // too large for one SM, or periodic faces
     if (variant == 6 && !pn_resident_supported(g, P)) return big;   // 3D, wider than 2048, or periodic faces
     return variant;
@@ -174,21 +287,31 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     const int nb = grid_for(nvec, g.sms);
     pn_fused_plan* fplan = nullptr;
     if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
-    if (scheme == 5 || scheme == 6) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu, pn_resident.cu); `iterations` is not a bound here
+    if (scheme == 5 || scheme == 6 || scheme == 8) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu, pn_resident.cu, k_cg_persist); `iterations` is not a bound here
         if (ev) cudaEventRecord(ev[0], st);
-        cudaError_t e5 = scheme == 5 ? pn_launch_cg_onchip(g, P, 1 << 30, st) : pn_launch_cg_resident(g, P, 1 << 30, st);
+        cudaError_t e5;
+        if (scheme == 5) e5 = pn_launch_cg_onchip(g, P, 1 << 30, st);
+        else if (scheme == 6) e5 = pn_launch_cg_resident(g, P, 1 << 30, st);
+        else {
+            e5 = cudaMemsetAsync(P.gbar, 0, sizeof(unsigned int), st);
+            int G = g.sms < PN_RESIDENT_MAX_CTAS ? g.sms : PN_RESIDENT_MAX_CTAS, mi = 1 << 30;
+            pn_geom gg = g;
+            pn_ptrs PP = P;
+            void* args[] = {(void*)&gg, (void*)&PP, (void*)&mi};
+            if (e5 == cudaSuccess) e5 = cudaLaunchCooperativeKernel((const void*)k_cg_persist, dim3(G), dim3(ST), args, 0, st);
+        }
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         *launches += 1;
         return e5;
     }
-    if (scheme == 7 || scheme == 8) {   // compacted unknowns (pn_compact.cu): two kernels per iteration / one persistent launch
+    if (scheme == 7 || scheme == 9) {   // compacted unknowns (pn_compact.cu): two kernels per iteration (7) / one persistent launch (9, internal)
         if (!compact) return cudaErrorInvalidValue;
         if (scheme == 7) return pn_launch_compact_inner(g, P, *compact, iterations, st, launches, ev);
         if (ev) cudaEventRecord(ev[0], st);
-        cudaError_t e8 = pn_launch_compact_persist(g, P, *compact, 1 << 30, st);
+        cudaError_t e9 = pn_launch_compact_persist(g, P, *compact, 1 << 30, st);
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         *launches += 1;
-        return e8;
+        return e9;
     }
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];   // periodic lateral faces: k_wrap_fix finishes kernel A
     cudaError_t e = cudaSuccess;

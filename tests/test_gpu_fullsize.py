@@ -122,6 +122,7 @@ def test_cfg4_full_512cubed_certificate(pn, oracle):
     info, fl, pf = certify(pn, oracle, net, h, 0, 1e-10)
     h.close()
     assert info.n_floating > 0 and info.n_solved > 0.5 * net.n_nodes
+    assert info.kernel_scheme == 3                      # the automatic choice at this size: the fused TMA kernel
 
 
 def test_cfg5_full_512cubed_certificate(pn, oracle):

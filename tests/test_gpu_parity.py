@@ -107,14 +107,17 @@ def test_cfg5_sibling(pn, oracle, direction):
 def test_cfg4_sibling_128(pn, oracle):
     """2^21 nodes, tol 1e-13: several tiles in x and y and several z chunks with default options."""
     from paper_1908_03301_b200 import inputs
-    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13)
+    net = inputs.cfg4_fbm_cut_3d(128, 128, 128)
+    auto, *_ = compare(pn, oracle, net, 0, tol=1e-13)
+    tma, *_ = compare(pn, oracle, net, 0, tol=1e-13, opts={pn.PN_OPT_KERNEL: 3})
+    assert auto.kernel_scheme == 8 and tma.kernel_scheme == 3
 
 
 # ---- ragged shapes, every direction, 2D and 3D, with and without dilution ------------------------
 @pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 31, 7), (130, 6, 3)])
 @pytest.mark.parametrize("direction", [0, 1, 2])
 @pytest.mark.parametrize("p", [1.0, 0.6])
-@pytest.mark.parametrize("kernel", [1, 3])
+@pytest.mark.parametrize("kernel", [1, 3, 8])
 def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
     """kernel 1 = reference two-kernel iteration, 3 = single fused TMA kernel per iteration (forced, whatever the size)."""
     from paper_1908_03301_b200 import inputs
@@ -125,7 +128,7 @@ def test_ragged_3d(pn, oracle, shape, direction, p, kernel):
 @pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (3, 64), (257, 31)])
 @pytest.mark.parametrize("direction", [0, 1])
 @pytest.mark.parametrize("p", [1.0, 0.7])
-@pytest.mark.parametrize("kernel", [1, 3, 6])
+@pytest.mark.parametrize("kernel", [1, 3, 6, 8])
 def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(shape[0], shape[1], 1, seed=11 + direction, p=p)
@@ -150,7 +153,7 @@ def test_tma_kernel_2d_wide(pn, oracle, kernel):
     compare(pn, oracle, net, 1, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("kernel", [1, 3])
+@pytest.mark.parametrize("kernel", [1, 3, 8])
 def test_kernel_variants(pn, oracle, kernel):
     """Both S4 kernels must pass the same parity bar (0 = automatic choice is what the other tests use)."""
     from paper_1908_03301_b200 import inputs
@@ -318,7 +321,7 @@ def test_error_paths(pn):
 def test_max_iters_status(pn):
     from paper_1908_03301_b200 import inputs
     net = inputs.cfg2_fbm_2d(128, 128)
-    for kernel in (1, 3):
+    for kernel in (1, 3, 8):
         info, *_ = gpu_solve(pn, net, 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40, pn.PN_OPT_KERNEL: kernel})
         assert info.status == pn.PN_MAX_ITERS
         assert 40 <= info.inner_iters <= 40 + 64
@@ -329,7 +332,7 @@ def test_deterministic(pn):
     """Fixed-order grid reductions: two solves of the same input agree bit for bit."""
     from paper_1908_03301_b200 import inputs
     net = inputs.cfg3_percolation_3d(40, 40, 40)
-    for kernel in (1, 3):
+    for kernel in (1, 3, 8):
         a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel})
         b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel})
         assert a[0].inner_iters == b[0].inner_iters
@@ -809,13 +812,13 @@ def test_compaction_policy_and_determinism(pn, oracle):
     assert auto.kernel_scheme == 7 and auto.n_unknowns < 0.45 * near.n_nodes
     dense = inputs.cfg5_stratified_3d(32, 32, 32)
     d, *_ = compare(pn, oracle, dense, 0)
-    assert d.kernel_scheme == 1                                # nothing to skip: a structured kernel (small lattice: the pair)
+    assert d.kernel_scheme == 8                                # nothing to skip: a structured kernel (small lattice: persistent)
     per, *_ = compare(pn, oracle, near, 0, periodic=True)
     assert per.kernel_scheme == 1                              # periodic faces: a structured kernel + k_wrap_fix
     forced, *_ = compare(pn, oracle, near, 0, opts={pn.PN_OPT_KERNEL: 3})
     assert forced.kernel_scheme == 3                           # an explicit kernel choice is honoured
     full, *_ = compare(pn, oracle, inputs.cfg4_fbm_cut_3d(48, 40, 36), 1, opts={pn.PN_OPT_COMPACT: 1})
-    assert full.kernel_scheme == 1                             # table larger than the workspace arrays: structured kernel
+    assert full.kernel_scheme == 8                             # table larger than the workspace arrays: structured kernel
     a = gpu_solve(pn, near, 0, 1e-10)
     b = gpu_solve(pn, near, 0, 1e-10)
     assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]
@@ -824,11 +827,12 @@ def test_compaction_policy_and_determinism(pn, oracle):
 
 
 def test_automatic_kernel_choice_by_size(pn, oracle):
-    """0 = automatic: one CTA (5) / resident 2D slabs (6) / the cache-fed pair up to 600 000 padded nodes (1) / the fused TMA
-    kernel above (3) -- all through the same parity bar."""
+    """0 = automatic: one CTA (5) / resident 2D slabs (6) / the persistent structured kernel up to 5 000 000 padded nodes (8; the
+    cache-fed pair, 1, with periodic faces) / the fused TMA kernel above (3: tests/test_gpu_fullsize.py) -- all through the
+    same parity bar."""
     from paper_1908_03301_b200 import inputs
     for net, d, want in ((inputs.cfg5_stratified_3d(16, 16, 16), 0, 5), (inputs.cfg2_fbm_2d(300, 200), 0, 6),
-                         (inputs.cfg5_stratified_3d(64, 64, 64), 2, 1), (inputs.cfg5_stratified_3d(96, 96, 80), 0, 3)):
+                         (inputs.cfg5_stratified_3d(64, 64, 64), 2, 8), (inputs.cfg5_stratified_3d(96, 96, 80), 0, 8)):
         info, *_ = compare(pn, oracle, net, d)
         assert info.kernel_scheme == want, (net.name, info.kernel_scheme)
 
