@@ -409,7 +409,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     CK(cudaMemsetAsync(&P.st->iters, 0, sizeof(int), s));   // buffer parity of the first residual = 0
     int scheme = pn_resolve_variant(g, P, ctx->variant);
     int fused = scheme == 3 || scheme == 6 || scheme == 8;   // deferred residual update + predicted beta (the state holds the measured r.r)
-    int bufmode = scheme == 3 ? 1 : ((scheme == 6 || scheme == 8) ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
+    int bufmode = (scheme == 3 || scheme == 8) ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -463,7 +463,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     const size_t vbytes = (size_t)g.npad * 4;
     CK(cudaMemsetAsync(P.xh, 0, vbytes, s));
     CK(cudaMemsetAsync(P.q, 0, vbytes, s));
-    if (scheme == 3) CK(cudaMemsetAsync(P.q2, 0, vbytes, s));
+    if (scheme == 3 || scheme == 8) CK(cudaMemsetAsync(P.q2, 0, vbytes, s));
     // p / p2 double as export staging (pn_get_pressures), halo planes included: clear them whole
     const size_t vhalo = ((size_t)g.npad + 2 * (size_t)g.plane) * 4;
     CK(cudaMemsetAsync(P.p - g.plane, 0, vhalo, s));
@@ -539,7 +539,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         rn = 0.0;
     } else if (rn > tol * nb) {
         const double delta2 = ctx->delta * ctx->delta;
-        const double xskip_min = (fused && scheme != 7 && scheme != 8 && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
+        const double xskip_min = (fused && scheme != 7 && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
         auto target_for = [&](double rn_true, double rr_true) {
             // proxy of the fp64 exit test in the scaled norm: ||r|| / ||r_hat|| measured at this replacement
             const double c = rn_true / sqrt(rr_true);

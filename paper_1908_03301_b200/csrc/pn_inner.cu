@@ -152,9 +152,19 @@ __device__ __forceinline__ void sp_grid_barrier(unsigned int* bar, unsigned int 
     __threadfence();   // acquire; also drops the SM's L1 lines, so that the plain loads that follow see the other CTAs' stores
 }
 
+// p_t at a node from the previous iteration's r, q, p there: the deferred residual update, recomputed wherever needed
+__device__ __forceinline__ float4 pnew4(const float* __restrict__ r, const float* __restrict__ q, const float* __restrict__ p,
+                                        long long n, float nal, float beta) {
+    return fma4(beta, ld4(p + n), fma4(nal, ld4(q + n), ld4(r + n)));
+}
+__device__ __forceinline__ float pnew1(const float* __restrict__ r, const float* __restrict__ q, const float* __restrict__ p,
+                                       long long n, float nal, float beta) {
+    return fmaf(beta, p[n], fmaf(nal, q[n], r[n]));
+}
+
 __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int max_launch_iters) {
     pn_state* st = P.st;
-    if (st->flag != PN_FLAG_RUN) return;   // same value in every CTA: nobody enters the barriers alone
+    if (st->flag != PN_FLAG_RUN) return;   // same value in every CTA: nobody enters the barrier alone
     __shared__ double red[4 * 32 + 8];
     __shared__ pn_state ls;                 // this CTA's copy of the iteration state
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -166,46 +176,61 @@ __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int 
     const long long v0 = min(per * c, nvec), v1 = min(v0 + per, nvec);
     const int px = g.px;
     const long long plane = g.plane;
+    const bool has_y = g.ny > 1;            // 2D lattices are held as nx x 1 x rows: no y bonds
     const float* __restrict__ wx = P.w[0];
     const float* __restrict__ wy = P.w[1];
     const float* __restrict__ wz = P.w[2];
-    float* __restrict__ r = P.r;
-    float* __restrict__ q = P.q;
-    float* __restrict__ p = P.p;
     unsigned int* bar = P.gbar;
     unsigned int bar_target = 0;
 
     for (int li = 0; li < max_launch_iters; ++li) {
         const int pin = li & 1;
+        const int par = ls.iters & 1;                               // buffers holding r_{t-1}, q_{t-1}, p_{t-1}
+        const float* __restrict__ r = par ? P.r2 : P.r;
+        const float* __restrict__ q = par ? P.q2 : P.q;
+        const float* __restrict__ p = par ? P.p2 : P.p;
+        float* __restrict__ r_out = par ? P.r : P.r2;
+        float* __restrict__ q_out = par ? P.q : P.q2;
+        float* __restrict__ p_out = par ? P.p : P.p2;
         const float al = (float)ls.alpha, nal = -al, beta = (float)ls.beta;
+        // x_hat every other iteration, exactly as in k_cg_fused_tma
+        const int xmode = ls.xpend ? 2 : ((ls.xskip_min > 0.0 && ls.beta >= ls.xskip_min) ? 0 : 1);
+        const float c2 = xmode == 2 ? (float)(ls.alpha2 / ls.beta_prev) : 0.f;
         double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
         for (long long v = v0 + tid; v < v1; v += ST) {
             const long long n = 4 * v;
-            const float4 qq = ld4(q + n), po = ld4(p + n);
-            const float4 rn = fma4(nal, qq, ld4(r + n));
-            st4(P.xh + n, fma4(al, po, ld4(P.xh + n)));
-            st4(r + n, rn);
-            st4(p + n, fma4(beta, po, rn));
-            a_rr += (double)(rn.x * rn.x + rn.y * rn.y + rn.z * rn.z + rn.w * rn.w);
-        }
-        __syncthreads();
-        if (tid == 0) { bar_target += G; sp_grid_barrier(bar, bar_target); }
-        __syncthreads();
-        for (long long v = v0 + tid; v < v1; v += ST) {
-            const long long n = 4 * v;
-            const float4 pn = ld4(p + n);
-            const float pl = p[n - 1], pr = p[n + 4];
-            const float4 pym = ld4(p + n - px), pyp = ld4(p + n + px), pzm = ld4(p + n - plane), pzp = ld4(p + n + plane);
-            const float4 gx = ld4(wx + n), gy = ld4(wy + n), gz = ld4(wz + n);
+            const float4 ro = ld4(r + n), po = ld4(p + n);
+            const float4 rn = fma4(nal, ld4(q + n), ro);
+            const float4 pn = fma4(beta, po, rn);
+            const float pl = pnew1(r, q, p, n - 1, nal, beta), pr = pnew1(r, q, p, n + 4, nal, beta);
+            const float4 pzm = pnew4(r, q, p, n - plane, nal, beta), pzp = pnew4(r, q, p, n + plane, nal, beta);
+            const float4 gx = ld4(wx + n), gz = ld4(wz + n), gzm = ld4(wz + n - plane);
             const float gxl = wx[n - 1];
-            const float4 gym = ld4(wy + n - px), gzm = ld4(wz + n - plane);
-            float4 qv;
-            qv.x = pn.x - (gxl * pl + gx.x * pn.y + gym.x * pym.x + gy.x * pyp.x + gzm.x * pzm.x + gz.x * pzp.x);
-            qv.y = pn.y - (gx.x * pn.x + gx.y * pn.z + gym.y * pym.y + gy.y * pyp.y + gzm.y * pzm.y + gz.y * pzp.y);
-            qv.z = pn.z - (gx.y * pn.y + gx.z * pn.w + gym.z * pym.z + gy.z * pyp.z + gzm.z * pzm.z + gz.z * pzp.z);
-            qv.w = pn.w - (gx.z * pn.z + gx.w * pr + gym.w * pym.w + gy.w * pyp.w + gzm.w * pzm.w + gz.w * pzp.w);
-            st4(q + n, qv);
-            const float4 rn = ld4(r + n);
+            float4 s;
+            s.x = gxl * pl + gx.x * pn.y + gzm.x * pzm.x + gz.x * pzp.x;
+            s.y = gx.x * pn.x + gx.y * pn.z + gzm.y * pzm.y + gz.y * pzp.y;
+            s.z = gx.y * pn.y + gx.z * pn.w + gzm.z * pzm.z + gz.z * pzp.z;
+            s.w = gx.z * pn.z + gx.w * pr + gzm.w * pzm.w + gz.w * pzp.w;
+            if (has_y) {
+                const float4 pym = pnew4(r, q, p, n - px, nal, beta), pyp = pnew4(r, q, p, n + px, nal, beta);
+                const float4 gy = ld4(wy + n), gym = ld4(wy + n - px);
+                s.x += gym.x * pym.x + gy.x * pyp.x;
+                s.y += gym.y * pym.y + gy.y * pyp.y;
+                s.z += gym.z * pym.z + gy.z * pyp.z;
+                s.w += gym.w * pym.w + gy.w * pyp.w;
+            }
+            const float4 qv = make_float4(pn.x - s.x, pn.y - s.y, pn.z - s.z, pn.w - s.w);
+            st4(r_out + n, rn);
+            st4(p_out + n, pn);
+            st4(q_out + n, qv);
+            if (xmode) {
+                float4 xn = fma4(al, po, ld4(P.xh + n));
+                if (xmode == 2)
+                    xn = make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
+                                     fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
+                st4(P.xh + n, xn);
+            }
+            a_rr += (double)(rn.x * rn.x + rn.y * rn.y + rn.z * rn.z + rn.w * rn.w);
             a_pq += (double)(pn.x * qv.x + pn.y * qv.y + pn.z * qv.z + pn.w * qv.w);
             a_rq += (double)(rn.x * qv.x + rn.y * qv.y + rn.z * qv.z + rn.w * qv.w);
             a_qq += (double)(qv.x * qv.x + qv.y * qv.y + qv.z * qv.z + qv.w * qv.w);
