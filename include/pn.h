@@ -100,7 +100,7 @@ enum {
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared
                                memory -- at most 7168 padded floats per array, no periodic faces --, 6 where it
-                               applies, 8 on other lattices of at most 5 000 000 padded nodes, else 3),
+                               applies, 8 on other lattices of at most 5 000 000 (3D) / 12 000 000 (2D) padded nodes, else 3),
                                1 = reference pair: S4 kernel reading neighbours through the caches + S5
                                kernel (kept as an independently written cross-check),
                                3 = ONE TMA-fed kernel per iteration (S4 + S5 + S6 fused),
@@ -109,8 +109,8 @@ enum {
                                at most 2048 wide, no periodic faces): ONE persistent cooperative launch per residual
                                replacement, every CTA keeping its slab on chip, grid barrier per iteration; else 3,
                                8 = any lattice without periodic faces: ONE persistent cooperative launch per residual
-                               replacement, vectors in HBM / L2, two grid barriers per iteration (for lattices that
-                               sit in the L2, where an iteration is bound by launches, not by HBM); with periodic faces: 1.
+                               replacement, neighbours through L1 / L2, one grid barrier per iteration (for lattices
+                               whose planes sit in the L2, where launch boundaries cost more than the re-reads); with periodic faces: 1.
                                (2 and 4 were round-1 experiments, since removed: PN_ERR_ARG)                   */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */

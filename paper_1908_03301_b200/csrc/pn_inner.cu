@@ -133,16 +133,16 @@ __global__ void __launch_bounds__(TPB) k_update(int nvec, pn_ptrs P) {
     }
 }
 
-// ---- the same iteration for SMALL lattices as ONE persistent cooperative launch per residual replacement -----------------
-// Below ~600 000 nodes an iteration is bound by launches, not by memory (12.5 us at 64^3 for the pair above, of which the
-// two kernels' work is a fraction; profiles/r02_small_lattices.md).  Here every CTA owns a fixed range of the lattice for the
-// whole launch; an iteration is two phases with the recurrences of the single-kernel scheme (deferred residual update,
-// predicted beta: pn_finish_F) separated by two grid barriers:
-//   phase U   r_t = r - alpha q ;  x_hat += alpha p ;  p_t = r_t + beta p ;  r_t.r_t              (own nodes)
-//   barrier   (the stencil reads other CTAs' p_t)
-//   phase S   q_t = p_t - W p_t, neighbours through L1 / L2 as in k_stencil_simple ;  p.q, r.q, q.q   (own nodes)
-//   barrier + every CTA adds the slots in the same fixed order and runs pn_finish_F on its own copy of the state
-// (k_cg_resident2d and k_cpersist work the same way).  Vectors live in one buffer each (P.r, P.q, P.p).
+// ---- the single-kernel iteration as ONE persistent cooperative launch per residual replacement, cache-fed -----------------
+// Below a few million nodes an iteration is bound by launch boundaries, not by memory (the pair above: 12 us at 64^3; the
+// fused TMA kernel: ~16 us of ring ramp + reduction tail per launch; profiles/r02_small_lattices.md).  Here every CTA owns a
+// fixed range of the lattice for the whole launch and runs the recurrences of k_cg_fused_tma (pn_fused_tma.cu) on it:
+//   r_t = r - alpha q ;  p_t = r_t + beta p  at the node AND, recomputed from their r, q, p, at its six neighbours (through
+//   L1 / L2: no shared-memory tiles) ;  x_hat every other iteration ;  q_t = p_t - W p_t ;  r.r, p.q, r.q, q.q
+//   ONE grid barrier; then every CTA adds the slots in the same fixed order and runs pn_finish_F on its own copy of the state
+// (k_cg_resident2d and k_cpersist work the same way).  r, q, p are double-buffered by iteration parity as in k_cg_fused_tma.
+// A two-phase form (update, barrier, stencil, barrier; single buffers) was measured first: 7.8 / 16.7 / 34.0 us at 64^3 /
+// 128^3 / 2048^2 against 6.5 / 16.1 / 28.5 us for this one.
 constexpr int ST = 1024;
 
 __device__ __forceinline__ void sp_grid_barrier(unsigned int* bar, unsigned int target) {
@@ -280,22 +280,24 @@ int grid_for(long long work_items, int sms) {
 
 // PN_OPT_KERNEL: 0 = automatic: the whole loop in one CTA when the lattice fits one SM's shared memory (5); the persistent
 // shared-memory-resident kernel for 2D lattices whose slabs fit all SMs (6); the persistent structured kernel above (8)
-// for the other lattices of at most PN_SMALL_LATTICE padded nodes (with periodic faces: the cache-fed pair, 1); else the
-// single fused TMA kernel (3).  Measured on B200 (profiles/r02_small_lattices.md), per iteration, persistent / pair /
-// fused: 7.8 / 12.2 / 15.3 us at 64^3, 10.7 / 19.3 / 19.1 at 96^3, 16.7 / - / 26.0 at 128^3, 33.9 / - / 43.1 at 160^3,
-// 69.6 / - / 61.0 at 192^3, 180 / - / 120 at 256^3; 2D: 14.9 / - / 27.1 at 1448^2, 34.0 / - / 34.3 at 2048^2.  The fused
-// kernel pays ~16 us of TMA ring ramp and reduction tail per launch but moves 40 instead of 52 bytes per node: it wins
-// once the lattice no longer sits in the L2 (from ~5 M nodes).
+// for the other lattices of at most PN_SMALL_LATTICE (3D) / PN_SMALL_LATTICE_2D padded nodes (with periodic faces: the
+// cache-fed pair, 1); else the single fused TMA kernel (3).  Measured on B200 (profiles/r02_small_lattices.md), per
+// iteration, persistent / fused TMA: 6.5 / 15.3 us at 64^3, 9.6 / 19.1 at 96^3, 16.1 / 26.0 at 128^3, 34.2 / 43.1 at 160^3,
+// 71.1 / 61.0 at 192^3; 2D: 12.0 / 27.1 at 1448^2, 28.5 / 34.3 at 2048^2, 61.9 / 75.2 at 3072^2, 109.1 / 107.9 at 4096^2.
+// The TMA kernel pays ~16 us of ring ramp and reduction tail per launch but fetches every value from L2 / HBM once per
+// tile; the persistent kernel re-reads the neighbours' r, q, p through L1 / L2, which is free while the lattice's planes
+// sit there and costs bandwidth beyond.
 // 1 = the pair on any lattice (independently written cross-check).  The two superseded schemes of round 1 (2: TMA S4
 // kernel + S5 kernel, 4: q recomputed) are gone; their write-ups remain in profiles/r01_tma_kernel.md and
 // profiles/r01_q_recompute_experiment.md.
-constexpr long long PN_SMALL_LATTICE = 5000000;
+constexpr long long PN_SMALL_LATTICE = 5000000;      // 3D
+constexpr long long PN_SMALL_LATTICE_2D = 12000000;  // 2D lattices (held as nx x 1 x rows)
 int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant) {
     const int big = pn_tma_supported() ? 3 : 1;
     if (variant == 0) {
         if (pn_onchip_supported(g)) return 5;
         if (pn_resident_supported(g, P)) return 6;
-        if (g.npad <= PN_SMALL_LATTICE) return (g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2])) ? 8 : 1;
+        if (g.npad <= (g.ny == 1 ? PN_SMALL_LATTICE_2D : PN_SMALL_LATTICE)) return (g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2])) ? 8 : 1;
         return big;
     }
     if (variant == 8 && !(g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2]))) return 1;   // periodic faces / no cooperative launch
