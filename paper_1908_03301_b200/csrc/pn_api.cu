@@ -555,7 +555,9 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         // duration, gaps and the no-op tail included); the two-kernel schemes keep per-launch events to split S4 from S5.
         // compacted unknowns: PN_OPT_GRAPH = 1 means the persistent cooperative launch (one per residual replacement);
         // 0 the two kernels of an iteration launched one by one
-        const int lscheme = (scheme == 7 && ctx->use_graph && g.coop) ? 9 : scheme;
+        // the fused TMA kernel likewise (internal code 10), unless periodic faces need k_wrap_fix between the iterations
+        const int lscheme = (scheme == 7 && ctx->use_graph && g.coop) ? 9
+                            : ((scheme == 3 && ctx->use_graph && g.coop && !any_wrap) ? 10 : scheme);
         const bool graph = ctx->use_graph && ctx->chunk > 1 && lscheme < 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme, cm, clong);
         const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);   // (scheme 7: two kernels, never with wrap)
         while (true) {
@@ -574,7 +576,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);
                 if (ran > 0) { t_stencil += ta; n_timed += ran; }
-            } else if (ctx->profile && (lscheme == 5 || lscheme == 6 || lscheme == 8 || lscheme == 9)) {   // one launch ran `ran` iterations (on chip / persistent)
+            } else if (ctx->profile && (lscheme == 5 || lscheme == 6 || lscheme >= 8)) {   // one launch ran `ran` iterations (on chip / persistent)
                 const int ran = h->iters - iters_seen;
                 float ta = 0.f;
                 cudaEventElapsedTime(&ta, ctx->pev[0], ctx->pev[1]);

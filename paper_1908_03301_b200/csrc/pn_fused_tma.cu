@@ -71,11 +71,26 @@ struct alignas(64) pn_fmaps {
     CUtensorMap wx_main, wx_slv, wy, wz;
 };
 
-template <class C>
+// PERSIST: the same kernel as ONE cooperative launch per fp64 residual replacement -- the iteration loop runs inside, the
+// last-block epilogue becomes a grid barrier after which every CTA adds the per-CTA sums in the same fixed order and runs
+// pn_finish_F on its own copy of the state (as k_cg_resident2d / k_cg_persist / k_cpersist do).  Saves the launch gap, the
+// state reads and the reduction tail of every iteration (~17 us of 868 at 512^3); not with periodic faces (k_wrap_fix).
+__device__ __forceinline__ void ft_grid_barrier(unsigned int* bar, unsigned int target) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
+    unsigned int v;
+    do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory"); } while (v < target);
+    __threadfence();
+}
+
+template <class C, bool PERSIST>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
-k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz) {
-    pn_state* st = P.st;
-    if (st->flag != PN_FLAG_RUN) return;
+k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz,
+               int max_launch_iters) {
+    pn_state* gst = P.st;
+    if (gst->flag != PN_FLAG_RUN) return;
+    __shared__ pn_state ls_;                 // PERSIST: this CTA's copy of the iteration state
+    __shared__ double red2[4 * 32 + 8];      // PERSIST: warp partials of the four sums
+    pn_state* st = PERSIST ? &ls_ : gst;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // The integer round trip on the base pointer makes every tile access a GENERIC load / store (the compiler can no longer
     // prove the shared address space); without it the compiler emits LDS / STS.  Measured, same box (profiles/
@@ -90,6 +105,20 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     double* red = reinterpret_cast<double*>(empty + C::S);   // 32 doubles + 4 totals
 
     const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s = 0; s < C::S; ++s) {
+            mbar_init(full + s, 1);
+            mbar_init(empty + s, C::NCONS / 32);
+        }
+        mbar_fence_init();
+        if (PERSIST) ls_ = *gst;
+    }
+    __syncthreads();
+    const int tiles = ntx * nty;
+    const int total = tiles * nchunks;
+    unsigned it = 0;                            // stage counter of this thread's role; runs on across iterations
+    unsigned int bar_target = 0;
+  for (int li = 0; li < max_launch_iters; ++li) {
     const float beta = (float)st->beta;
     const float al = (float)st->alpha;          // alpha_{t-1} (0 right after a residual replacement)
     const float nal = -al;
@@ -102,24 +131,12 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     float* __restrict__ r_out = par ? P.r : P.r2;
     float* __restrict__ q_out = par ? P.q : P.q2;
     float* __restrict__ p_out = par ? P.p : P.p2;
-
-    if (tid == 0) {
-        for (int s = 0; s < C::S; ++s) {
-            mbar_init(full + s, 1);
-            mbar_init(empty + s, C::NCONS / 32);
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    const int tiles = ntx * nty;
-    const int total = tiles * nchunks;
     double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
 
     if (tid >= C::NCONS) {
         // ================= producer warp: one elected lane issues every TMA load =================
         if (tid == C::NCONS) {
-            unsigned it = 0;
+            if (PERSIST) asm volatile("fence.proxy.async;" ::: "memory");   // other CTAs' stores of the last iteration -> this one's TMA loads
             for (int item = blockIdx.x; item < total; item += gridDim.x) {
                 const int chunk = item / tiles, t = item - chunk * tiles;
                 const int tyi = t / ntx, txi = t - tyi * ntx;
@@ -177,7 +194,6 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
         const int hb = has_halo ? hidx / 128 : 0;
         const int hrow = has_halo ? (((hidx >> 6) & 1) ? C::RH - 1 : 0) : 0;
         const int hc4 = hidx & 63;
-        unsigned it = 0;
         for (int item = blockIdx.x; item < total; item += gridDim.x) {
             const int chunk = item / tiles, t = item - chunk * tiles;
             const int tyi = t / ntx, txi = t - tyi * ntx;
@@ -287,19 +303,57 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
             }
         }
     }
-    // ---- the four sums: warp -> block -> grid; the last block computes alpha_t and beta_{t+1} ----
-    a_rr = pn_block_sum(a_rr, red);
-    a_pq = pn_block_sum(a_pq, red);
-    a_rq = pn_block_sum(a_rq, red);
-    a_qq = pn_block_sum(a_qq, red);
-    const double v4[4] = {a_rr, a_pq, a_rq, a_qq};
-    if (pn_grid_sum<4>(v4, P.slots, &st->ticket, red, red + 32)) {
-        if (threadIdx.x == 0) {
-            if (g.wrap[0] | g.wrap[1] | g.wrap[2]) {   // periodic faces: k_wrap_fix adds the wrap bonds' part and finishes
-                st->part[0] = red[32]; st->part[1] = red[33]; st->part[2] = red[34]; st->part[3] = red[35];
-            } else pn_finish_F(st, red[32], red[33], red[34], red[35]);
+    if (!PERSIST) {
+        // ---- the four sums: warp -> block -> grid; the last block computes alpha_t and beta_{t+1} ----
+        a_rr = pn_block_sum(a_rr, red);
+        a_pq = pn_block_sum(a_pq, red);
+        a_rq = pn_block_sum(a_rq, red);
+        a_qq = pn_block_sum(a_qq, red);
+        const double v4[4] = {a_rr, a_pq, a_rq, a_qq};
+        if (pn_grid_sum<4>(v4, P.slots, &st->ticket, red, red + 32)) {
+            if (threadIdx.x == 0) {
+                if (g.wrap[0] | g.wrap[1] | g.wrap[2]) {   // periodic faces: k_wrap_fix adds the wrap bonds' part and finishes
+                    st->part[0] = red[32]; st->part[1] = red[33]; st->part[2] = red[34]; st->part[3] = red[35];
+                } else pn_finish_F(st, red[32], red[33], red[34], red[35]);
+            }
         }
+        return;
     }
+    // ---- PERSIST: warp -> CTA -> slots [parity][CTA][4] -> grid barrier -> every CTA adds the slots in the same order ----
+    {
+        const int lane = tid & 31, wid = tid >> 5, pin = li & 1, G = (int)gridDim.x, c = (int)blockIdx.x;
+        a_rr = pn_warp_sum(a_rr); a_pq = pn_warp_sum(a_pq); a_rq = pn_warp_sum(a_rq); a_qq = pn_warp_sum(a_qq);
+        if (lane == 0) { red2[wid] = a_rr; red2[32 + wid] = a_pq; red2[64 + wid] = a_rq; red2[96 + wid] = a_qq; }
+        __syncthreads();
+        if (wid == 0) {
+            constexpr int NW = C::NTHREADS / 32;
+            double* my = P.slots + ((size_t)pin * PN_MAX_BLOCKS + c) * 4;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double v = pn_warp_sum(lane < NW ? red2[32 * k + lane] : 0.0);
+                if (lane == 0) my[k] = v;
+            }
+            if (lane == 0) { bar_target += G; ft_grid_barrier(P.gbar, bar_target); }
+            __syncwarp();
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+            const double2* sl = reinterpret_cast<const double2*>(P.slots + (size_t)pin * PN_MAX_BLOCKS * 4);
+            double2 va[(PN_RESIDENT_MAX_CTAS + 31) / 32], vb[(PN_RESIDENT_MAX_CTAS + 31) / 32];
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) {
+                const int b = lane + 32 * u;
+                va[u] = b < G ? __ldcg(sl + 2 * b) : make_double2(0.0, 0.0);
+                vb[u] = b < G ? __ldcg(sl + 2 * b + 1) : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int u = 0; u < (PN_RESIDENT_MAX_CTAS + 31) / 32; ++u) { t0 += va[u].x; t1 += va[u].y; t2 += vb[u].x; t3 += vb[u].y; }
+            t0 = pn_warp_sum(t0); t1 = pn_warp_sum(t1); t2 = pn_warp_sum(t2); t3 = pn_warp_sum(t3);
+            if (lane == 0) pn_finish_F(&ls_, t0, t1, t2, t3);
+        }
+        __syncthreads();
+        if (ls_.flag != PN_FLAG_RUN) break;
+    }
+  }
+    if (PERSIST && blockIdx.x == 0 && tid == 0) *gst = ls_;
 }
 
 // ---- host side ----------------------------------------------------------------------------------------
@@ -321,15 +375,25 @@ bool build_maps(pn_fmaps* M, const pn_geom& g, const pn_ptrs& P) {
 }
 
 template <class C>
-cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, cudaStream_t st) {
+cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, int max_launch_iters, cudaStream_t st) {
     const int ntx = (g.px + C::TXW - 1) / C::TXW, nty = (g.ny + C::TY - 1) / C::TY;
     const int sms = g.sms;
     const int lz = choose_lz(g.nz, ntx * nty, sms, 44.0, 24.0);   // two extra planes of r, q, p per chunk
     const int nchunks = (g.nz + lz - 1) / lz;
     const long long total = (long long)ntx * nty * nchunks;
     const int nb = (int)(total < sms ? total : sms);
-    k_cg_fused_tma<C><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(M, g, P, ntx, nty, nchunks, lz);
-    return cudaGetLastError();
+    if (max_launch_iters <= 0) {   // one iteration per launch
+        k_cg_fused_tma<C, false><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(M, g, P, ntx, nty, nchunks, lz, 1);
+        return cudaGetLastError();
+    }
+    cudaError_t e = cudaMemsetAsync(P.gbar, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+    pn_fmaps MM = M;
+    pn_geom gg = g;
+    pn_ptrs PP = P;
+    int a_ntx = ntx, a_nty = nty, a_nch = nchunks, a_lz = lz, a_mi = max_launch_iters;
+    void* args[] = {(void*)&MM, (void*)&gg, (void*)&PP, (void*)&a_ntx, (void*)&a_nty, (void*)&a_nch, (void*)&a_lz, (void*)&a_mi};
+    return cudaLaunchCooperativeKernel((const void*)k_cg_fused_tma<C, true>, dim3(nb), dim3(C::NTHREADS), args, C::SMEM_BYTES, st);
 }
 
 typedef FCfg<1, 8, true, 3> FCfg3D;    // 256 x 8 tile, y halo, 3 stages
@@ -341,9 +405,11 @@ bool pn_tma_supported() { return get_encoder() != nullptr; }
 
 // cudaFuncSetAttribute is per device: pn_create calls this with the handle's device current
 cudaError_t pn_fused_init_device() {
-    cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
+    return e;
 }
 
 struct pn_fused_plan {
@@ -364,6 +430,8 @@ bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P
 
 void pn_fused_plan_free(pn_fused_plan* pl) { delete pl; }
 
-cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st) {
-    return pl->is2d ? launch_cfg<FCfg2D>(g, P, pl->maps, st) : launch_cfg<FCfg3D>(g, P, pl->maps, st);
+// max_launch_iters <= 0: ONE iteration (the launch a CUDA graph replays); > 0: a cooperative launch that iterates up to the
+// next trigger (no periodic faces)
+cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int max_launch_iters) {
+    return pl->is2d ? launch_cfg<FCfg2D>(g, P, pl->maps, max_launch_iters, st) : launch_cfg<FCfg3D>(g, P, pl->maps, max_launch_iters, st);
 }

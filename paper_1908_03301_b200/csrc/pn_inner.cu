@@ -313,7 +313,15 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     const int nvec = (int)(g.npad / 4);
     const int nb = grid_for(nvec, g.sms);
     pn_fused_plan* fplan = nullptr;
-    if (scheme == 3 && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
+    if ((scheme == 3 || scheme == 10) && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
+    if (scheme == 10) {   // the fused TMA kernel as one persistent cooperative launch up to the next trigger (internal code)
+        if (ev) cudaEventRecord(ev[0], st);
+        cudaError_t e10 = pn_launch_cg_fused(fplan, g, P, st, 1 << 30);
+        if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
+        pn_fused_plan_free(fplan);
+        *launches += 1;
+        return e10;
+    }
     if (scheme == 5 || scheme == 6 || scheme == 8) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu, pn_resident.cu, k_cg_persist); `iterations` is not a bound here
         if (ev) cudaEventRecord(ev[0], st);
         cudaError_t e5;

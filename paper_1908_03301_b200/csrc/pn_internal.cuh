@@ -247,7 +247,7 @@ cudaError_t pn_launch_export_cls(const pn_geom& g, const pn_ptrs& P, signed char
 struct pn_fused_plan;
 bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P);
 void pn_fused_plan_free(pn_fused_plan* pl);
-cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st);
+cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int max_launch_iters = 0);
 
 // periodic lateral faces (pn_wrap.cu): the wrap bonds' part of q and of the dot products; finishes alpha / beta
 cudaError_t pn_launch_wrap_fix(const pn_geom& g, const pn_ptrs& P, int fused, cudaStream_t st);

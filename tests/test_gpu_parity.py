@@ -536,23 +536,47 @@ def test_anisotropic_fbm_both_directions(pn, oracle):
 @pytest.mark.parametrize("kernel", [1, 3])
 def test_graph_replay_is_bit_identical(pn, kernel):
     """PN_OPT_GRAPH: replaying chunks from a CUDA graph launches the same kernels on the same data -- pressures,
-    fluxes and iteration counts are identical to direct launches; the graph is reused across solves of one handle."""
+    fluxes and iteration counts are identical to direct launches; the graph is reused across solves of one handle.
+    (The fused TMA kernel is replayed from a graph only with periodic faces -- otherwise PN_OPT_GRAPH = 1 means its
+    persistent cooperative form, whose sums are grouped differently: test_persistent_launch_of_the_tma_kernel.)"""
     from paper_1908_03301_b200 import inputs
     net = inputs.cfg3_percolation_3d(48, 48, 48)
-    a = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 1})
-    b = gpu_solve(pn, net, 0, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 0})
+    base = {pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_LATERAL: 1 if kernel == 3 else 0}
+    a = gpu_solve(pn, net, 0, 1e-10, opts={**base, pn.PN_OPT_GRAPH: 1})
+    b = gpu_solve(pn, net, 0, 1e-10, opts={**base, pn.PN_OPT_GRAPH: 0})
     assert a[0].inner_iters == b[0].inner_iters and a[0].outer_cycles == b[0].outer_cycles
     assert np.array_equal(a[1], b[1]) and a[3] == b[3]
     assert a[4] == b[4]                                   # same launch count
     h = pn.Network(net.nx, net.ny, net.nz)
-    h.set_option(pn.PN_OPT_KERNEL, kernel)
+    for k, v in base.items():
+        h.set_option(k, v)
     h.set_conductances(net.gx, net.gy, net.gz)
     for d in (0, 1, 0, 2):                                # direction changes force a re-capture
         h.solve(d, 1e-10)
         P = h.pressures().cpu().numpy()
-        ref = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_GRAPH: 0})
+        ref = gpu_solve(pn, net, d, 1e-10, opts={**base, pn.PN_OPT_GRAPH: 0})
         assert np.array_equal(P, ref[1])
     h.close()
+
+
+def test_persistent_launch_of_the_tma_kernel(pn, oracle):
+    """PN_OPT_KERNEL = 3 with PN_OPT_GRAPH = 1 (default) and no periodic faces: the fused TMA kernel runs as ONE cooperative
+    launch per residual replacement.  Same parity bar, the iteration count of the launch-per-iteration form to a few per
+    cent (the dot products are grouped per CTA instead of per block), far fewer launches, and bit-reproducible."""
+    from paper_1908_03301_b200 import inputs
+    for net, d in ((inputs.cfg4_fbm_cut_3d(64, 64, 64), 0), (inputs.iid_diluted(300, 20, 70, seed=5, p=0.75), 2),
+                   (inputs.iid_diluted(2100, 40, 1, seed=9, p=1.0), 1)):
+        on, *_ = compare(pn, oracle, net, d, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0})
+        off, *_ = compare(pn, oracle, net, d, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0, pn.PN_OPT_GRAPH: 0})
+        assert on.kernel_scheme == off.kernel_scheme == 3
+        assert abs(on.inner_iters - off.inner_iters) <= 0.05 * off.inner_iters + 5
+        a = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0})
+        b = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0})
+        c = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0, pn.PN_OPT_GRAPH: 0})
+        assert a[0].inner_iters == b[0].inner_iters and np.array_equal(a[1], b[1]) and a[3] == b[3]
+        assert a[4] < c[4] / 5                            # launches
+    info, *_ = gpu_solve(pn, inputs.cfg2_fbm_2d(300, 200), 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40, pn.PN_OPT_KERNEL: 3})
+    assert info.status == pn.PN_MAX_ITERS and info.inner_iters == 40
 
 
 @pytest.mark.parametrize("maker,direction,periodic", [
