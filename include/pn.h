@@ -45,7 +45,8 @@ enum {
     PN_ERR_VALUE = -3,          /* negative, NaN or Inf conductance on an in-lattice bond           */
     PN_ERR_WORKSPACE = -4,      /* workspace missing, misaligned (256 B) or too small               */
     PN_ERR_CUDA = -5,           /* a CUDA call failed (sticky; pn_last_error has the text)          */
-    PN_ERR_BREAKDOWN = -6       /* CG breakdown: p.Ap <= 0 or non-finite                            */
+    PN_ERR_BREAKDOWN = -6,      /* CG breakdown: p.Ap <= 0 or non-finite                            */
+    PN_ERR_TOO_LARGE = -7       /* pn_dissipation_noalloc: more than PN_NOALLOC_MAX_NODES nodes     */
 };
 
 /* node classes written by pn_get_classes (S8(c) steps 2-3) */
@@ -216,6 +217,32 @@ int pn_flux(pn_ctx* ctx, double* q_in, double* q_out, double* g_eff, double* k_e
  * its error is quadratic in the error of the pressures where g_eff's (boundary fluxes) is linear: a cross-check that
  * holds to ~1e-12 already at a 1e-10 residual (S8(c) consequence (iv)).  HOST pointer.  Needs a finished pn_solve. */
 int pn_dissipation(pn_ctx* ctx, double* g_e);
+
+/* The same dissipation sum WITHOUT a handle, a workspace or any allocation -- for callers that may not allocate
+ * device memory (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ *   g_e = sum over all bonds g (P_i - P_j)^2        (energy identity of P:53 with eq.(4), dP = 1)
+ * over the network AS THE CALLER HOLDS IT: gx, gy, gz in the layout of pn_set_conductances (forward-bond convention,
+ * gz NULL iff nz == 1), `pressures` in the layout of pn_get_pressures (nx*ny*nz doubles).  Bit b of `periodic_mask`
+ * (b = 0, 1, 2 for x, y, z): that axis wraps around, the forward entry of its last node being the bond back to the
+ * first (PN_OPT_LATERAL = 1 with solve axis a: every bit but a); other forward entries that leave the lattice are
+ * ignored.  With the pressures of a finished pn_solve the result equals pn_dissipation's up to the order of the sum
+ * (pinned clusters are at one pressure: their bonds add exact zeros).
+ * ALL pointers are DEVICE pointers on `device`, owned by the caller; `g_e` receives ONE double, written on
+ * `cuda_stream` (NULL = the legacy default stream): the call only enqueues (one 4-byte memset + one kernel) and does
+ * not synchronise.  The sum is taken over fixed chunks of 8192 nodes whose partial sums are added in chunk order: the
+ * value does not depend on the GPU or on block scheduling.
+ * Scratch: the chunk sums and an arrival counter live in a file-scope `static __device__` array of
+ * PN_NOALLOC_MAX_NODES / 8192 + 32 doubles (about 256 KB), which every GPU that loads the library holds until exit.
+ * Limit: nx*ny*nz <= PN_NOALLOC_MAX_NODES (2^28 = 268 435 456 nodes; 512^3 is 2^27), else PN_ERR_TOO_LARGE and nothing
+ * is enqueued.  The array is shared by every call in the process: calls that may OVERLAP on one GPU (different
+ * streams, different host threads) race on it and must be ordered by the caller; calls on one stream are safe.  The
+ * counter is cleared at the start of every call; the chunk sums need no clearing (every chunk in use is rewritten).
+ * Calls no cudaMalloc / cudaFree and no allocating library routine (first use on a device: cudaGetSymbolAddress and
+ * cudaDeviceGetAttribute).  Errors: PN_ERR_ARG (null pointer, bad shape or mask, gz given for nz == 1 or missing for
+ * nz > 1), PN_ERR_TOO_LARGE, PN_ERR_CUDA. */
+#define PN_NOALLOC_MAX_NODES 268435456LL
+int pn_dissipation_noalloc(int nx, int ny, int nz, const float* gx, const float* gy, const float* gz,
+                           const double* pressures, int periodic_mask, double* g_e, int device, void* cuda_stream);
 
 /* Tuning knobs (PN_OPT_*).  PN_ERR_ARG on an unknown key or out-of-range value. */
 int pn_set_option(pn_ctx* ctx, int key, double value);

@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpn.so")
-SOURCES = ["pn_api.cu", "pn_setup.cu", "pn_outer.cu", "pn_inner.cu", "pn_fused_tma.cu", "pn_resident.cu", "pn_compact.cu", "pn_chain.cu", "pn_wrap.cu", "pn_onchip.cu"]
+SOURCES = ["pn_api.cu", "pn_setup.cu", "pn_outer.cu", "pn_inner.cu", "pn_fused_tma.cu", "pn_resident.cu", "pn_compact.cu", "pn_chain.cu", "pn_wrap.cu", "pn_onchip.cu", "pn_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "pn_internal.cuh"), os.path.join(CSRC, "pn_tma.cuh"), os.path.join(CSRC, "pn_chain.cuh"), os.path.join(HERE, "..", "include", "pn.h")]
 
 

@@ -285,6 +285,7 @@ const char* pn_strerror(int code) {
         case PN_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
         case PN_ERR_CUDA: return "CUDA error";
         case PN_ERR_BREAKDOWN: return "conjugate-gradient breakdown";
+        case PN_ERR_TOO_LARGE: return "more nodes than PN_NOALLOC_MAX_NODES (268435456): the fixed scratch array of pn_dissipation_noalloc does not hold them";
         default: return "unknown code";
     }
 }

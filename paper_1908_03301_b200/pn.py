@@ -23,6 +23,8 @@ LIB_PATH = os.path.join(HERE, "libpn.so")
 
 PN_OK, PN_NO_SPANNING_CLUSTER, PN_MAX_ITERS = 0, 1, 2
 PN_ERR_ARG, PN_ERR_STATE, PN_ERR_VALUE, PN_ERR_WORKSPACE, PN_ERR_CUDA, PN_ERR_BREAKDOWN = -1, -2, -3, -4, -5, -6
+PN_ERR_TOO_LARGE = -7
+PN_NOALLOC_MAX_NODES = 1 << 28
 (PN_OPT_MAX_ITERS, PN_OPT_DELTA, PN_OPT_X0, PN_OPT_CHUNK, PN_OPT_SKIP_LABEL, PN_OPT_KERNEL, PN_OPT_PROFILE,
  PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER, PN_OPT_REUSE_LABELS, PN_OPT_COMPACT, PN_OPT_CONTRACT) = range(14)
 CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CLASS_FLOATING = range(6)
@@ -31,7 +33,7 @@ CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CL
 SYMBOLS = ("pn_workspace_bytes", "pn_create", "pn_set_conductances", "pn_solve", "pn_get_pressures",
            "pn_get_classes", "pn_flux", "pn_set_option", "pn_launch_count", "pn_destroy", "pn_strerror",
            "pn_last_error", "pn_residual_history", "pn_dissipation", "pn_update_conductances",
-           "pn_replace_conductances")
+           "pn_replace_conductances", "pn_dissipation_noalloc")
 
 
 class PnInfo(ctypes.Structure):
@@ -116,6 +118,8 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.pn_launch_count.restype = ctypes.c_longlong
     lib.pn_dissipation.argtypes = [vp, dp]
     lib.pn_dissipation.restype = ctypes.c_int
+    lib.pn_dissipation_noalloc.argtypes = [ctypes.c_int] * 3 + [vp, vp, vp, vp, ctypes.c_int, vp, ctypes.c_int, vp]
+    lib.pn_dissipation_noalloc.restype = ctypes.c_int
     lib.pn_residual_history.argtypes = [vp, dp, ctypes.c_int]
     lib.pn_residual_history.restype = ctypes.c_int
     lib.pn_destroy.argtypes = [vp]
@@ -306,3 +310,33 @@ class Network:
 
     def __exit__(self, *exc):
         self.close()
+
+
+def dissipation_noalloc(gx, gy, gz, pressures, out, periodic_mask: int = 0, stream=None) -> None:
+    """pn_dissipation_noalloc: G_E of the network the CALLER holds, written to `out[0]` on the stream; allocates nothing.
+
+    gx, gy, gz (None for 2D): float32 CUDA tensors of shape (nz, ny, nx) as given to `Network.set_conductances`;
+    `pressures`: float64 CUDA tensor of that shape (`Network.pressures()`); `out`: float64 CUDA tensor with >= 1 element,
+    allocated by the caller.  Only enqueues: read `out` after synchronising the stream.  At most PN_NOALLOC_MAX_NODES
+    nodes (PnError with PN_ERR_TOO_LARGE beyond); overlapping calls on one GPU share one scratch array and race."""
+    import torch
+    lib = load_library()
+    for name, t, dt in (("gx", gx, torch.float32), ("gy", gy, torch.float32), ("gz", gz, torch.float32),
+                        ("pressures", pressures, torch.float64), ("out", out, torch.float64)):
+        if t is None and name == "gz":
+            continue
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dt and t.is_contiguous()):
+            raise TypeError(f"{name}: contiguous CUDA tensor of {dt} expected")
+    if pressures.dim() != 3 or out.numel() < 1:
+        raise ValueError("pressures: shape (nz, ny, nx); out: at least one element")
+    nz, ny, nx = pressures.shape
+    for name, t in (("gx", gx), ("gy", gy), ("gz", gz)):
+        if t is not None and t.numel() != pressures.numel():
+            raise ValueError(f"{name}: {pressures.numel()} elements expected")
+    if stream is None:
+        stream = torch.cuda.current_stream(pressures.device)
+    rc = lib.pn_dissipation_noalloc(nx, ny, nz, gx.data_ptr(), gy.data_ptr(), gz.data_ptr() if gz is not None else None,
+                                    pressures.data_ptr(), int(periodic_mask), out.data_ptr(), pressures.device.index,
+                                    ctypes.c_void_p(stream.cuda_stream))
+    if rc != PN_OK:
+        raise PnError(rc, strerror(rc))

@@ -54,7 +54,7 @@ def test_workspace_bytes(lib):
 
 def test_strerror(lib):
     from paper_1908_03301_b200 import pn
-    texts = {c: pn.strerror(c) for c in range(-6, 3)}
+    texts = {c: pn.strerror(c) for c in range(-7, 3)}
     assert len(set(texts.values())) == len(texts)
     assert pn.strerror(12345) == "unknown code"
 
@@ -105,3 +105,22 @@ def test_product_does_not_import_oracle():
         if f.endswith((".py", ".c")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1908_03301_b200" not in text.replace("(`paper_1908_03301_b200/`)", ""), f
+
+
+def test_noalloc_argument_errors(lib):
+    """pn_dissipation_noalloc refuses bad shapes and sizes beyond its fixed scratch array before any CUDA call."""
+    from paper_1908_03301_b200 import pn
+    p = ctypes.c_void_p(256)
+    f = lib.pn_dissipation_noalloc
+    assert f(0, 4, 4, p, p, p, p, 0, p, 0, None) == pn.PN_ERR_ARG
+    assert f(4, 4, 4, None, p, p, p, 0, p, 0, None) == pn.PN_ERR_ARG
+    assert f(4, 4, 4, p, p, p, p, 0, None, 0, None) == pn.PN_ERR_ARG
+    assert f(4, 4, 4, p, p, None, p, 0, p, 0, None) == pn.PN_ERR_ARG          # 3D without gz
+    assert f(4, 4, 1, p, p, p, p, 0, p, 0, None) == pn.PN_ERR_ARG             # 2D with gz
+    assert f(4, 4, 4, p, p, p, p, 8, p, 0, None) == pn.PN_ERR_ARG             # mask has three bits
+    assert f(4, 4, 4, p, p, p, p, 0, p, -1, None) == pn.PN_ERR_ARG
+    assert f(1024, 1024, 257, p, p, p, p, 0, p, 0, None) == pn.PN_ERR_TOO_LARGE
+    assert f(1 << 20, 1 << 20, 1, p, p, None, p, 0, p, 0, None) == pn.PN_ERR_TOO_LARGE
+    assert f(2147483647, 2147483647, 2147483647, p, p, p, p, 0, p, 0, None) == pn.PN_ERR_TOO_LARGE
+    assert pn.PN_NOALLOC_MAX_NODES == 1024 * 1024 * 256
+    assert "PN_NOALLOC_MAX_NODES" in pn.strerror(pn.PN_ERR_TOO_LARGE)
