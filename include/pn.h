@@ -109,9 +109,9 @@ enum {
                                6 = 2D lattices whose rows / SMs slabs fit the SMs' shared memory (about 1.2 M nodes,
                                at most 2048 wide, no periodic faces): ONE persistent cooperative launch per residual
                                replacement, every CTA keeping its slab on chip, grid barrier per iteration; else 3,
-                               8 = any lattice without periodic faces: ONE persistent cooperative launch per residual
+                               8 = any lattice, periodic faces included: ONE persistent cooperative launch per residual
                                replacement, neighbours through L1 / L2, one grid barrier per iteration (for lattices
-                               whose planes sit in the L2, where launch boundaries cost more than the re-reads); with periodic faces: 1.
+                               whose planes sit in the L2, where launch boundaries cost more than the re-reads).
                                (2 and 4 were round-1 experiments, since removed: PN_ERR_ARG)                   */
     PN_OPT_PROFILE = 6,     /* 1: record CUDA events around every S4 / S5 launch and report the
                                summed kernel times in pn_info (default 0)                           */

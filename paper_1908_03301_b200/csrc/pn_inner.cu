@@ -162,6 +162,10 @@ __device__ __forceinline__ float pnew1(const float* __restrict__ r, const float*
     return fmaf(beta, p[n], fmaf(nal, q[n], r[n]));
 }
 
+// WRAP: periodic lateral faces.  A node on a wrapping face has one more bond, to the node on the
+// opposite face, weight in the face array ww (pn_setup.cu k_wrap_weights; zero on pad columns); its p_t is recomputed from
+// r, q, p there like any other neighbour's: no second kernel (k_wrap_fix, pn_wrap.cu) and no second barrier.
+template <bool WRAP>
 __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int max_launch_iters) {
     pn_state* st = P.st;
     if (st->flag != PN_FLAG_RUN) return;   // same value in every CTA: nobody enters the barrier alone
@@ -218,6 +222,31 @@ __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int 
                 s.y += gym.y * pym.y + gy.y * pyp.y;
                 s.z += gym.z * pym.z + gy.z * pyp.z;
                 s.w += gym.w * pym.w + gy.w * pyp.w;
+            }
+            if (WRAP) {
+                const long long row = n / px;
+                const int i0 = (int)(n - row * px), j = (int)(row % g.ny), k = (int)(row / g.ny);
+                if (g.wrap[0]) {
+                    const int last = g.nx - 1, e = last - i0;
+                    const float w0 = P.ww[0][j + (long long)g.ny * k];
+                    if (i0 == 0) s.x += w0 * pnew1(r, q, p, n + last, nal, beta);
+                    if (e >= 0 && e < 4) {
+                        const float t = w0 * pnew1(r, q, p, n + e - last, nal, beta);
+                        if (e == 0) s.x += t; else if (e == 1) s.y += t; else if (e == 2) s.z += t; else s.w += t;
+                    }
+                }
+                if (g.wrap[1] && (j == 0 || j == g.ny - 1)) {
+                    const long long sp = (long long)(g.ny - 1) * px;
+                    const float4 w1 = ld4(P.ww[1] + i0 + (long long)px * k);
+                    const float4 pp = pnew4(r, q, p, j == 0 ? n + sp : n - sp, nal, beta);
+                    s.x += w1.x * pp.x; s.y += w1.y * pp.y; s.z += w1.z * pp.z; s.w += w1.w * pp.w;
+                }
+                if (g.wrap[2] && (k == 0 || k == g.nz - 1)) {
+                    const long long sp = (long long)(g.nz - 1) * plane;
+                    const float4 w2 = ld4(P.ww[2] + i0 + (long long)px * j);
+                    const float4 pp = pnew4(r, q, p, k == 0 ? n + sp : n - sp, nal, beta);
+                    s.x += w2.x * pp.x; s.y += w2.y * pp.y; s.z += w2.z * pp.z; s.w += w2.w * pp.w;
+                }
             }
             const float4 qv = make_float4(pn.x - s.x, pn.y - s.y, pn.z - s.z, pn.w - s.w);
             st4(r_out + n, rn);
@@ -280,8 +309,8 @@ int grid_for(long long work_items, int sms) {
 
 // PN_OPT_KERNEL: 0 = automatic: the whole loop in one CTA when the lattice fits one SM's shared memory (5); the persistent
 // shared-memory-resident kernel for 2D lattices whose slabs fit all SMs (6); the persistent structured kernel above (8)
-// for the other lattices of at most PN_SMALL_LATTICE (3D) / PN_SMALL_LATTICE_2D padded nodes (with periodic faces: the
-// cache-fed pair, 1); else the single fused TMA kernel (3).  Measured on B200 (profiles/r02_small_lattices.md), per
+// for the other lattices of at most PN_SMALL_LATTICE (3D) / PN_SMALL_LATTICE_2D padded nodes (periodic faces included:
+// its WRAP instantiation; without cooperative launch: the cache-fed pair, 1); else the single fused TMA kernel (3).  Measured on B200 (profiles/r02_small_lattices.md), per
 // iteration, persistent / fused TMA: 6.5 / 15.3 us at 64^3, 9.6 / 19.1 at 96^3, 16.1 / 26.0 at 128^3, 34.2 / 43.1 at 160^3,
 // 71.1 / 61.0 at 192^3; 2D: 12.0 / 27.1 at 1448^2, 28.5 / 34.3 at 2048^2, 61.9 / 75.2 at 3072^2, 109.1 / 107.9 at 4096^2.
 // The TMA kernel pays ~16 us of ring ramp and reduction tail per launch but fetches every value from L2 / HBM once per
@@ -297,10 +326,10 @@ int pn_resolve_variant(const pn_geom& g, const pn_ptrs& P, int variant) {
     if (variant == 0) {
         if (pn_onchip_supported(g)) return 5;
         if (pn_resident_supported(g, P)) return 6;
-        if (g.npad <= (g.ny == 1 ? PN_SMALL_LATTICE_2D : PN_SMALL_LATTICE)) return (g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2])) ? 8 : 1;
+        if (g.npad <= (g.ny == 1 ? PN_SMALL_LATTICE_2D : PN_SMALL_LATTICE)) return g.coop ? 8 : 1;
         return big;
     }
-    if (variant == 8 && !(g.coop && !(g.wrap[0] | g.wrap[1] | g.wrap[2]))) return 1;   // periodic faces / no cooperative launch
+    if (variant == 8 && !g.coop) return 1;   // no cooperative launch on this device
     if (variant == 5 && !pn_onchip_supported(g)) return big;   // too large for one SM, or periodic faces
     if (variant == 6 && !pn_resident_supported(g, P)) return big;   // 3D, wider than 2048, or periodic faces
     return variant;
@@ -333,7 +362,8 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
             pn_geom gg = g;
             pn_ptrs PP = P;
             void* args[] = {(void*)&gg, (void*)&PP, (void*)&mi};
-            if (e5 == cudaSuccess) e5 = cudaLaunchCooperativeKernel((const void*)k_cg_persist, dim3(G), dim3(ST), args, 0, st);
+            const void* fn = (g.wrap[0] | g.wrap[1] | g.wrap[2]) ? (const void*)k_cg_persist<true> : (const void*)k_cg_persist<false>;
+            if (e5 == cudaSuccess) e5 = cudaLaunchCooperativeKernel(fn, dim3(G), dim3(ST), args, 0, st);
         }
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         *launches += 1;

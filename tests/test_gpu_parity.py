@@ -442,7 +442,7 @@ def test_peeling_automatic_policy(pn, oracle):
 @pytest.mark.parametrize("shape", [(17, 9, 5), (5, 17, 9), (9, 5, 17), (33, 2, 7), (12, 6, 2)])
 @pytest.mark.parametrize("direction", [0, 1, 2])
 @pytest.mark.parametrize("p", [1.0, 0.6])
-@pytest.mark.parametrize("kernel", [1, 3])
+@pytest.mark.parametrize("kernel", [1, 3, 8])
 def test_periodic_ragged_3d(pn, oracle, shape, direction, p, kernel):
     """All three kernel schemes; lateral axes of length 2 (a doubled bond) included."""
     from paper_1908_03301_b200 import inputs
@@ -454,14 +454,14 @@ def test_periodic_ragged_3d(pn, oracle, shape, direction, p, kernel):
 
 @pytest.mark.parametrize("shape", [(19, 13), (13, 19), (64, 3), (257, 31)])
 @pytest.mark.parametrize("direction", [0, 1])
-@pytest.mark.parametrize("kernel", [1, 3])
+@pytest.mark.parametrize("kernel", [1, 3, 8])
 def test_periodic_ragged_2d(pn, oracle, shape, direction, kernel):
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(shape[0], shape[1], 1, seed=13 + direction, p=0.75)
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
 
 
-@pytest.mark.parametrize("kernel", [3])
+@pytest.mark.parametrize("kernel", [3, 8])
 @pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
 def test_periodic_multi_tile(pn, oracle, shape, direction, kernel):
     from paper_1908_03301_b200 import inputs
@@ -472,7 +472,8 @@ def test_periodic_multi_tile(pn, oracle, shape, direction, kernel):
 def test_periodic_config_siblings(pn, oracle):
     from paper_1908_03301_b200 import inputs
     compare(pn, oracle, inputs.cfg2_fbm_2d(256, 256), 0, periodic=True)
-    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13, periodic=True)    # automatic: fused TMA kernel
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(128, 128, 128), 0, tol=1e-13, periodic=True)    # automatic: persistent kernel, WRAP form
+    compare(pn, oracle, inputs.cfg4_fbm_cut_3d(96, 80, 72), 1, periodic=True, opts={pn.PN_OPT_KERNEL: 3})   # fused TMA kernel + k_wrap_fix
     info, P, fl, ref = compare(pn, oracle, inputs.cfg3_percolation_3d(64, 64, 64), 0, periodic=True)
     from oracle import pn_oracle as po
     net = inputs.cfg3_percolation_3d(64, 64, 64)
@@ -711,7 +712,7 @@ def test_onchip_scheme_options(pn, oracle):
     on, *_ = compare(pn, oracle, net, 0, opts={pn.PN_OPT_PEEL: 1})
     assert on.n_peeled > 0 and on.kernel_scheme == 5
     per, *_ = compare(pn, oracle, net, 0, periodic=True)
-    assert per.kernel_scheme == 1                       # periodic faces on a small lattice: the cache-fed pair + k_wrap_fix
+    assert per.kernel_scheme == 8                       # periodic faces on a small lattice: the persistent kernel's WRAP form
     big, *_ = compare(pn, oracle, inputs.cfg3_percolation_3d(24, 24, 24, p=0.4), 0, opts={pn.PN_OPT_KERNEL: 5})
     assert big.kernel_scheme == 3                       # 24^3 does not fit: falls back
     a = gpu_solve(pn, net, 0, 1e-10)
@@ -838,7 +839,7 @@ def test_compaction_policy_and_determinism(pn, oracle):
     d, *_ = compare(pn, oracle, dense, 0)
     assert d.kernel_scheme == 8                                # nothing to skip: a structured kernel (small lattice: persistent)
     per, *_ = compare(pn, oracle, near, 0, periodic=True)
-    assert per.kernel_scheme == 1                              # periodic faces: a structured kernel + k_wrap_fix
+    assert per.kernel_scheme == 8                              # periodic faces: a structured kernel (wrap bonds inside it)
     forced, *_ = compare(pn, oracle, near, 0, opts={pn.PN_OPT_KERNEL: 3})
     assert forced.kernel_scheme == 3                           # an explicit kernel choice is honoured
     full, *_ = compare(pn, oracle, inputs.cfg4_fbm_cut_3d(48, 40, 36), 1, opts={pn.PN_OPT_COMPACT: 1})
@@ -851,8 +852,8 @@ def test_compaction_policy_and_determinism(pn, oracle):
 
 
 def test_automatic_kernel_choice_by_size(pn, oracle):
-    """0 = automatic: one CTA (5) / resident 2D slabs (6) / the persistent structured kernel up to 5 000 000 padded nodes (8; the
-    cache-fed pair, 1, with periodic faces) / the fused TMA kernel above (3: tests/test_gpu_fullsize.py) -- all through the
+    """0 = automatic: one CTA (5) / resident 2D slabs (6) / the persistent structured kernel up to 5 000 000 padded nodes (8; periodic
+    faces included) / the fused TMA kernel above (3: tests/test_gpu_fullsize.py) -- all through the
     same parity bar."""
     from paper_1908_03301_b200 import inputs
     for net, d, want in ((inputs.cfg5_stratified_3d(16, 16, 16), 0, 5), (inputs.cfg2_fbm_2d(300, 200), 0, 6),
