@@ -92,6 +92,7 @@ bool make_layout(int nx, int ny, int nz, layout* L) {
     g.wrap[0] = g.wrap[1] = g.wrap[2] = 0;
     g.sms = 0;
     g.coop = 0;
+    g.tile = 0;
     if (g.npad + 2 * g.plane >= (1ll << 31)) return false;
     L->halo = (size_t)g.plane;
     const size_t vec = (size_t)g.npad + 2 * L->halo;   // elements of a padded array with its two halo planes
@@ -256,6 +257,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
         case PN_OPT_CONTRACT: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->contract = (int)value; return PN_OK;
+        case PN_OPT_TILE: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->g.tile = (int)value; return PN_OK;
         case PN_OPT_COMPACT: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->compact = (int)value; return PN_OK;
         case PN_OPT_REUSE_LABELS: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->reuse_labels = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;
@@ -327,7 +329,7 @@ int pn_set_conductances(pn_ctx* ctx, const float* gx, const float* gy, const flo
 static bool same_geom(const pn_geom& a, const pn_geom& b) {
     return a.nx == b.nx && a.ny == b.ny && a.nz == b.nz && a.px == b.px && a.plane == b.plane && a.npad == b.npad &&
            a.n == b.n && a.dir == b.dir && a.n_a == b.n_a && a.stride_a == b.stride_a && a.wrap[0] == b.wrap[0] &&
-           a.wrap[1] == b.wrap[1] && a.wrap[2] == b.wrap[2] && a.sms == b.sms;
+           a.wrap[1] == b.wrap[1] && a.wrap[2] == b.wrap[2] && a.sms == b.sms && a.tile == b.tile;
 }
 
 static int read_state(pn_ctx* ctx) {

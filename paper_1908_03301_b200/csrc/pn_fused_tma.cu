@@ -31,7 +31,7 @@ namespace {
 
 using namespace pn_tma;
 
-template <int NBX_, int TY_, bool HAS_Y_, int S_>
+template <int NBX_, int TY_, bool HAS_Y_, int S_, int BOXW_ = 256>
 struct FCfg {
     static constexpr int NBX = NBX_, TY = TY_, S = S_;
     static constexpr bool HAS_Y = HAS_Y_;
@@ -40,14 +40,16 @@ struct FCfg {
     // (512^3); on the 2D tile it was 3.1 % slower with generic shared-memory accesses and is 0.7 % faster now that the 2D
     // tile uses LDS / STS (see the kernel's first lines)
     static constexpr bool BAR_END = true;
-    static constexpr int BOXW = 256;                       // TMA box limit per dimension
+    static constexpr int BOXW = BOXW_;                     // nodes per box row (256 = the TMA box limit per dimension)
+    static constexpr int LPR = BOXW / 4;                   // consumer lanes per box row (whole warps)
+    static_assert(BOXW % 128 == 0 && BOXW <= 256, "box rows of whole warps");
     static constexpr int TXW = BOXW * NBX;                 // tile width in nodes
     static constexpr int RH = TY + (HAS_Y ? 2 : 0);        // rows of r, q, p and p_new including the y halo
     static constexpr int RWY = TY + (HAS_Y ? 1 : 0);       // rows of the wy box (backward row included)
     static constexpr int W = TXW + 8;                      // p_new ring row: 4 pad + tile + 4 pad floats
-    static constexpr int NCONS = 64 * NBX * TY;            // consumer threads: one float4 of nodes each
+    static constexpr int NCONS = LPR * NBX * TY;           // consumer threads: one float4 of nodes each
     static constexpr int NTHREADS = NCONS + 32;            // + one producer warp
-    static constexpr int NHALO4 = HAS_Y ? 2 * 64 * NBX : 0;  // float4s in the two halo rows
+    static constexpr int NHALO4 = HAS_Y ? 2 * LPR * NBX : 0;  // float4s in the two halo rows
     // stage layout (floats): three haloed vectors, then the weights
     static constexpr int VEC = NBX * RH * BOXW + 2 * a32(RH * 4);   // main boxes, left sliver, right sliver
     static constexpr int V_SL = NBX * RH * BOXW;
@@ -82,10 +84,18 @@ __device__ __forceinline__ void ft_grid_barrier(unsigned int* bar, unsigned int 
     __threadfence();
 }
 
-template <class C, bool PERSIST>
+// NARROW (single-box tiles only): the lattice's width is cut into ntx EQUAL tiles of tw <= 256 nodes (tw a multiple of 4) instead
+// of 256-wide ones with a narrow remainder; the TMA boxes are tw wide (rows land in shared memory with pitch tw), lanes beyond
+// tw idle.  A tile step costs ~1.4 us whatever its width against 1.9 us of memory time for a full 256 x 8 tile, so a narrow
+// remainder tile is nearly as expensive as a full one: equal tiles (320^3: 259 -> 252 us) and, more so, the 128 x 16 tile for
+// widths that fill 256-wide tiles badly (252 -> 230 us; FCfg3DN below) keep more of every step's lanes busy.
+template <class C, bool PERSIST, bool NARROW>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
 k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz,
-               int max_launch_iters) {
+               int max_launch_iters, int tw) {
+    static_assert(!NARROW || C::NBX == 1, "equal narrow tiles: one box per tile");
+    const int bw = NARROW ? tw : C::BOXW;        // pitch of a box row in shared memory = tile width
+    const int txw = NARROW ? tw : C::TXW;
     pn_state* gst = P.st;
     if (gst->flag != PN_FLAG_RUN) return;
     __shared__ pn_state ls_;                 // PERSIST: this CTA's copy of the iteration state
@@ -140,9 +150,12 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
             for (int item = blockIdx.x; item < total; item += gridDim.x) {
                 const int chunk = item / tiles, t = item - chunk * tiles;
                 const int tyi = t / ntx, txi = t - tyi * ntx;
-                const int x0 = txi * C::TXW, y0 = tyi * C::TY, k0 = chunk * lz;
+                const int x0 = txi * txw, y0 = tyi * C::TY, k0 = chunk * lz;
                 const int k1 = min(k0 + lz, g.nz);
                 const int yh = y0 - (C::HAS_Y ? 1 : 0);
+                const unsigned b_rqp = NARROW ? 3u * (unsigned)(C::RH * bw + 2 * C::RH * 4) * 4u : C::B_RQP;
+                const unsigned b_w = NARROW ? (unsigned)(C::TY * bw + C::TY * 4 + (C::HAS_Y ? C::RWY * bw : 0)) * 4u : C::B_W;
+                const unsigned b_wz = NARROW ? (unsigned)(C::TY * bw) * 4u : C::B_WZ;
                 for (int kk = k0 - 2; kk < k1; ++kk, ++it) {
                     const int s = it % C::S;
                     const unsigned ph = (it / C::S) & 1u;
@@ -150,7 +163,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     float* sg = stages + s * C::STAGE_FLOATS;
                     const bool has_w = kk >= k0;
                     const bool has_wz = kk >= k0 - 1;
-                    mbar_expect_tx(full + s, C::B_RQP + (has_w ? C::B_W : 0u) + (has_wz ? C::B_WZ : 0u));
+                    mbar_expect_tx(full + s, b_rqp + (has_w ? b_w : 0u) + (has_wz ? b_wz : 0u));
                     const int zp = kk + 2;   // plane kk+1 (+1: the tensor maps start at the leading halo plane)
                     const int zw = kk + 1;   // plane kk
 #pragma unroll
@@ -160,7 +173,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                         for (int b = 0; b < C::NBX; ++b)
                             tma_load_3d(sv + b * C::RH * C::BOXW, &maps.v_main[v][par], x0 + b * C::BOXW, yh, zp, full + s);
                         tma_load_3d(sv + C::V_SL, &maps.v_slv[v][par], x0 - 4, yh, zp, full + s);
-                        tma_load_3d(sv + C::V_SR, &maps.v_slv[v][par], x0 + C::TXW, yh, zp, full + s);
+                        tma_load_3d(sv + C::V_SR, &maps.v_slv[v][par], x0 + txw, yh, zp, full + s);
                     }
                     if (has_w) {
 #pragma unroll
@@ -182,25 +195,26 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     } else {
         // ================= consumer warps ==========================================================
         const int lane = tid & 31;
-        const int tx = tid % (64 * C::NBX), ty = tid / (64 * C::NBX);
-        const int b = tx >> 6, c4 = tx & 63;
+        const int tx = tid % (C::LPR * C::NBX), ty = tid / (C::LPR * C::NBX);
+        const int b = tx / C::LPR, c4 = tx % C::LPR;
         const int rrow = ty + (C::HAS_Y ? 1 : 0);               // own row in the haloed arrays
         const int rcol = 4 + b * C::BOXW + c4 * 4;              // own column in a ring row
-        const int own_main = (b * C::RH + rrow) * C::BOXW + c4 * 4;   // own float4 inside the r / q / p main boxes
-        const int own_ty = (b * C::TY + ty) * C::BOXW + c4 * 4;       // own float4 inside the wx / wz boxes
+        const int own_main = (b * C::RH + rrow) * bw + c4 * 4;   // own float4 inside the r / q / p main boxes
+        const int own_ty = (b * C::TY + ty) * bw + c4 * 4;       // own float4 inside the wx / wz boxes
+        const bool act = !NARROW || c4 * 4 < tw;                 // lanes beyond a narrow tile's width idle
         // the float4 of the two halo rows this thread also owns in phase A (the LAST warps take them)
         const int hidx = tid - (C::NCONS - C::NHALO4);
         const bool has_halo = C::HAS_Y && hidx >= 0;
-        const int hb = has_halo ? hidx / 128 : 0;
-        const int hrow = has_halo ? (((hidx >> 6) & 1) ? C::RH - 1 : 0) : 0;
-        const int hc4 = hidx & 63;
+        const int hb = has_halo ? hidx / (2 * C::LPR) : 0;
+        const int hrow = has_halo ? (((hidx / C::LPR) & 1) ? C::RH - 1 : 0) : 0;
+        const int hc4 = hidx % C::LPR;
         for (int item = blockIdx.x; item < total; item += gridDim.x) {
             const int chunk = item / tiles, t = item - chunk * tiles;
             const int tyi = t / ntx, txi = t - tyi * ntx;
-            const int x0 = txi * C::TXW, y0 = tyi * C::TY, k0 = chunk * lz;
+            const int x0 = txi * txw, y0 = tyi * C::TY, k0 = chunk * lz;
             const int k1 = min(k0 + lz, g.nz);
             const int x = x0 + b * C::BOXW + c4 * 4, y = y0 + ty;
-            const bool inb = (x < g.px) && (y < g.ny);
+            const bool inb = act && (x < g.px) && (y < g.ny);
             const long long nrow = (long long)y * g.px + x;
             float4 wzm = make_float4(0.f, 0.f, 0.f, 0.f);
             float4 r_cur = make_float4(0.f, 0.f, 0.f, 0.f);     // r_t on the own float4 of plane kk
@@ -224,7 +238,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     const float4 ro = lds4(sg + C::R_ + own_main);      // r_{t-1}
                     r_nxt = fma4(nal, lds4(sg + C::Q_ + own_main), ro);
                     const float4 pn = fma4(beta, po, r_nxt);
-                    *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
+                    if (act) *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
                     if (kk + 1 >= k0 && kk + 1 < k1 && inb) {
                         const long long n = (long long)(kk + 1) * g.plane + nrow;
                         __stcs(reinterpret_cast<float4*>(r_out + n), r_nxt);
@@ -239,8 +253,8 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                         a_rr += (double)dot4(r_nxt, r_nxt);
                     }
                 }
-                if (has_halo) {
-                    const int o = (hb * C::RH + hrow) * C::BOXW + hc4 * 4;
+                if (has_halo && (!NARROW || hc4 * 4 < tw)) {
+                    const int o = (hb * C::RH + hrow) * bw + hc4 * 4;
                     const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
                     *reinterpret_cast<float4*>(rw + hrow * C::W + 4 + hb * C::BOXW + hc4 * 4) = fma4(beta, lds4(sg + C::P_ + o), rn);
                 }
@@ -248,7 +262,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     const int side = tid / C::RH, row = tid - side * C::RH;
                     const int o = (side ? C::V_SR : C::V_SL) + row * 4;
                     const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
-                    *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + C::TXW : 0)) = fma4(beta, lds4(sg + C::P_ + o), rn);
+                    *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + txw : 0)) = fma4(beta, lds4(sg + C::P_ + o), rn);
                 }
                 if (!C::BAR_END) bar_consumers(C::NCONS);
                 // ---- phase C: q_t(kk) = p_t - W p_t from the ring, weights from the stage.  Of plane kk+1, written just above,
@@ -267,7 +281,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     float gxl = __shfl_up_sync(0xffffffffu, gx.w, 1);
                     if (lane == 0) {
                         if (c4 != 0) gxl = sg[C::WX + own_ty - 1];
-                        else if (b != 0) gxl = sg[C::WX + ((b - 1) * C::TY + ty) * C::BOXW + C::BOXW - 1];
+                        else if (b != 0) gxl = sg[C::WX + ((b - 1) * C::TY + ty) * C::BOXW + C::BOXW - 1];   // (b != 0: never NARROW)
                         else gxl = sg[C::WX_SL + ty * 4 + 3];
                     }
                     const float4 gz = lds4(sg + C::WZ + own_ty);
@@ -278,8 +292,8 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     q.w = gx.z * pc.z + gx.w * pr + wzm.w * pzm.w + gz.w * pzp.w;
                     if (C::HAS_Y) {
                         const float4 pym = lds4(r0 - C::W), pyp = lds4(r0 + C::W);
-                        const int oy = (b * C::RWY + ty) * C::BOXW + c4 * 4;   // row ty of the wy box = lattice row y-1
-                        const float4 gym = lds4(sg + C::WY + oy), gy = lds4(sg + C::WY + oy + C::BOXW);
+                        const int oy = (b * C::RWY + ty) * bw + c4 * 4;   // row ty of the wy box = lattice row y-1
+                        const float4 gym = lds4(sg + C::WY + oy), gy = lds4(sg + C::WY + oy + bw);
                         q.x += gym.x * pym.x + gy.x * pyp.x;
                         q.y += gym.y * pym.y + gy.y * pyp.y;
                         q.z += gym.z * pym.z + gy.z * pyp.z;
@@ -357,33 +371,45 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
 }
 
 // ---- host side ----------------------------------------------------------------------------------------
+// width of the (equal) x tiles: 256-wide boxes per tile unless one box covers a tile and the width does not fill the last one
+template <class C>
+int tile_width(const pn_geom& g) {
+    if (C::NBX != 1 || g.px % C::BOXW == 0) return C::TXW;
+    const int ntx = (g.px + C::BOXW - 1) / C::BOXW;
+    return ((g.px + ntx - 1) / ntx + 3) / 4 * 4;
+}
+
 template <class C>
 bool build_maps(pn_fmaps* M, const pn_geom& g, const pn_ptrs& P) {
     const long long h = g.plane;
+    const int bw = C::NBX == 1 ? tile_width<C>(g) : C::BOXW;
     const float* vec[3][2] = {{P.r, P.r2}, {P.q, P.q2}, {P.p, P.p2}};
     bool ok = true;
     for (int v = 0; v < 3; ++v)
         for (int bsel = 0; bsel < 2; ++bsel) {
-            ok &= make_map(&M->v_main[v][bsel], g, vec[v][bsel] - h, C::BOXW, C::RH);
+            ok &= make_map(&M->v_main[v][bsel], g, vec[v][bsel] - h, bw, C::RH);
             ok &= make_map(&M->v_slv[v][bsel], g, vec[v][bsel] - h, 4, C::RH);
         }
-    ok &= make_map(&M->wx_main, g, P.w[0] - h, C::BOXW, C::TY);
+    ok &= make_map(&M->wx_main, g, P.w[0] - h, bw, C::TY);
     ok &= make_map(&M->wx_slv, g, P.w[0] - h, 4, C::TY);
-    ok &= make_map(&M->wy, g, P.w[1] - h, C::BOXW, C::RWY);
-    ok &= make_map(&M->wz, g, P.w[2] - h, C::BOXW, C::TY);
+    ok &= make_map(&M->wy, g, P.w[1] - h, bw, C::RWY);
+    ok &= make_map(&M->wz, g, P.w[2] - h, bw, C::TY);
     return ok;
 }
 
 template <class C>
 cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, int max_launch_iters, cudaStream_t st) {
-    const int ntx = (g.px + C::TXW - 1) / C::TXW, nty = (g.ny + C::TY - 1) / C::TY;
+    const int tw = tile_width<C>(g);
+    const bool narrow = tw != C::TXW;
+    const int ntx = (g.px + tw - 1) / tw, nty = (g.ny + C::TY - 1) / C::TY;
     const int sms = g.sms;
     const int lz = choose_lz(g.nz, ntx * nty, sms, 44.0, 24.0);   // two extra planes of r, q, p per chunk
     const int nchunks = (g.nz + lz - 1) / lz;
     const long long total = (long long)ntx * nty * nchunks;
     const int nb = (int)(total < sms ? total : sms);
     if (max_launch_iters <= 0) {   // one iteration per launch
-        k_cg_fused_tma<C, false><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(M, g, P, ntx, nty, nchunks, lz, 1);
+        if (narrow) k_cg_fused_tma<C, false, C::NBX == 1><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(M, g, P, ntx, nty, nchunks, lz, 1, tw);
+        else k_cg_fused_tma<C, false, false><<<nb, C::NTHREADS, C::SMEM_BYTES, st>>>(M, g, P, ntx, nty, nchunks, lz, 1, tw);
         return cudaGetLastError();
     }
     cudaError_t e = cudaMemsetAsync(P.gbar, 0, sizeof(unsigned int), st);
@@ -391,13 +417,22 @@ cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, in
     pn_fmaps MM = M;
     pn_geom gg = g;
     pn_ptrs PP = P;
-    int a_ntx = ntx, a_nty = nty, a_nch = nchunks, a_lz = lz, a_mi = max_launch_iters;
-    void* args[] = {(void*)&MM, (void*)&gg, (void*)&PP, (void*)&a_ntx, (void*)&a_nty, (void*)&a_nch, (void*)&a_lz, (void*)&a_mi};
-    return cudaLaunchCooperativeKernel((const void*)k_cg_fused_tma<C, true>, dim3(nb), dim3(C::NTHREADS), args, C::SMEM_BYTES, st);
+    int a_ntx = ntx, a_nty = nty, a_nch = nchunks, a_lz = lz, a_mi = max_launch_iters, a_tw = tw;
+    void* args[] = {(void*)&MM, (void*)&gg, (void*)&PP, (void*)&a_ntx, (void*)&a_nty, (void*)&a_nch, (void*)&a_lz, (void*)&a_mi, (void*)&a_tw};
+    const void* fn = narrow ? (const void*)k_cg_fused_tma<C, true, C::NBX == 1> : (const void*)k_cg_fused_tma<C, true, false>;
+    return cudaLaunchCooperativeKernel(fn, dim3(nb), dim3(C::NTHREADS), args, C::SMEM_BYTES, st);
 }
 
 typedef FCfg<1, 8, true, 3> FCfg3D;    // 256 x 8 tile, y halo, 3 stages
+typedef FCfg<1, 16, true, 3, 128> FCfg3DN;   // 128 x 16 tile for widths that fill 256-wide tiles badly (e.g. 320, 384)
 typedef FCfg<8, 1, false, 4> FCfg2D;   // 2048 x 1 tile (lattices held as nx x 1 x ny), 4 stages
+
+// fraction of the consumer lanes of a tiling that hold lattice nodes
+template <class C>
+double lane_efficiency(const pn_geom& g) {
+    const int ntx = (g.px + C::TXW - 1) / C::TXW, nty = (g.ny + C::TY - 1) / C::TY;
+    return ((double)g.px / ((double)ntx * C::TXW)) * ((double)g.ny / ((double)nty * C::TY));
+}
 
 }  // namespace
 
@@ -405,24 +440,34 @@ bool pn_tma_supported() { return get_encoder() != nullptr; }
 
 // cudaFuncSetAttribute is per device: pn_create calls this with the handle's device current
 cudaError_t pn_fused_init_device() {
-    cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3D, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
     return e;
 }
 
 struct pn_fused_plan {
     pn_fmaps maps;
-    bool is2d;
+    int kind;      // 0: 2D tile, 1: 256 x 8, 2: 128 x 16
 };
 
 bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P) {
     if (!get_encoder()) return false;
     pn_fused_plan* pl = new (std::nothrow) pn_fused_plan;
     if (!pl) return false;
-    pl->is2d = (g.ny == 1);
-    const bool ok = pl->is2d ? build_maps<FCfg2D>(&pl->maps, g, P) : build_maps<FCfg3D>(&pl->maps, g, P);
+    // 3D: the 128 x 16 tile where it fills its lanes at least 8 % better than the 256 x 8 one, which is the faster of the two on
+    // widths both fill (512^3: 0.861 against 0.884 ms per iteration; 256^3: 113.8 against 115.2 us).  Measured with the tile
+    // forced either way (profiles/r02_small_lattices.md): 320^3 252 -> 230 us, 384^3 392 -> 371 us, 260^3 161 -> 143 us
+    pl->kind = g.ny == 1 ? 0 : (g.tile ? g.tile : (lane_efficiency<FCfg3DN>(g) > 1.08 * lane_efficiency<FCfg3D>(g) ? 2 : 1));
+    const bool ok = pl->kind == 0 ? build_maps<FCfg2D>(&pl->maps, g, P)
+                                  : (pl->kind == 1 ? build_maps<FCfg3D>(&pl->maps, g, P) : build_maps<FCfg3DN>(&pl->maps, g, P));
     if (!ok) { delete pl; return false; }
     *out = pl;
     return true;
@@ -433,5 +478,6 @@ void pn_fused_plan_free(pn_fused_plan* pl) { delete pl; }
 // max_launch_iters <= 0: ONE iteration (the launch a CUDA graph replays); > 0: a cooperative launch that iterates up to the
 // next trigger (no periodic faces)
 cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int max_launch_iters) {
-    return pl->is2d ? launch_cfg<FCfg2D>(g, P, pl->maps, max_launch_iters, st) : launch_cfg<FCfg3D>(g, P, pl->maps, max_launch_iters, st);
+    if (pl->kind == 0) return launch_cfg<FCfg2D>(g, P, pl->maps, max_launch_iters, st);
+    return pl->kind == 1 ? launch_cfg<FCfg3D>(g, P, pl->maps, max_launch_iters, st) : launch_cfg<FCfg3DN>(g, P, pl->maps, max_launch_iters, st);
 }

@@ -26,7 +26,8 @@ PN_ERR_ARG, PN_ERR_STATE, PN_ERR_VALUE, PN_ERR_WORKSPACE, PN_ERR_CUDA, PN_ERR_BR
 PN_ERR_TOO_LARGE = -7
 PN_NOALLOC_MAX_NODES = 1 << 28
 (PN_OPT_MAX_ITERS, PN_OPT_DELTA, PN_OPT_X0, PN_OPT_CHUNK, PN_OPT_SKIP_LABEL, PN_OPT_KERNEL, PN_OPT_PROFILE,
- PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER, PN_OPT_REUSE_LABELS, PN_OPT_COMPACT, PN_OPT_CONTRACT) = range(14)
+ PN_OPT_PEEL, PN_OPT_LATERAL, PN_OPT_GRAPH, PN_OPT_XDEFER, PN_OPT_REUSE_LABELS, PN_OPT_COMPACT, PN_OPT_CONTRACT,
+ PN_OPT_TILE) = range(15)
 CLASS_INLET, CLASS_OUTLET, CLASS_SOLVED, CLASS_INLET_ONLY, CLASS_OUTLET_ONLY, CLASS_FLOATING = range(6)
 
 # every symbol include/pn.h declares (tests check that the library exports each of them)

@@ -135,14 +135,20 @@ def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("kernel", [3])
-@pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
-def test_tma_kernel_multi_tile(pn, oracle, shape, direction, kernel):
-    """Lattices wider than one 256-node TMA box and taller than one 8-row tile: x and y halos between
-    tiles, several z chunks, ragged tails in all three directions."""
+@pytest.mark.parametrize("tile", [0, 1, 2])
+@pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0), ((256, 33, 9), 0),
+                                             ((130, 40, 21), 1)])
+def test_tma_kernel_multi_tile(pn, oracle, shape, direction, tile):
+    """Lattices wider than one TMA box and taller than one tile: x and y halos between tiles, several z chunks, ragged
+    tails in all three directions.  Both 3D tiles (PN_OPT_TILE: 256 x 8 and 128 x 16 nodes; 0 = automatic); widths that do
+    not fill their last tile are cut into EQUAL narrower tiles (260 -> 2 x 132 or 3 x 88; 300 -> 2 x 152 or 3 x 100;
+    520 -> 3 x 176 or 5 x 104; 130 -> 1 x 132 or 2 x 68), 256 is the one exact fit."""
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(*shape, seed=5, p=0.75)
-    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
+    info, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_TILE: tile})
+    assert info.kernel_scheme == 3
+    one, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_TILE: tile, pn.PN_OPT_GRAPH: 0})
+    assert one.kernel_scheme == 3                       # the same tiles, one launch per iteration
 
 
 @pytest.mark.parametrize("kernel", [3, 6])
@@ -461,12 +467,12 @@ def test_periodic_ragged_2d(pn, oracle, shape, direction, kernel):
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
 
 
-@pytest.mark.parametrize("kernel", [3, 8])
+@pytest.mark.parametrize("kernel,tile", [(3, 1), (3, 2), (8, 0)])
 @pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
-def test_periodic_multi_tile(pn, oracle, shape, direction, kernel):
+def test_periodic_multi_tile(pn, oracle, shape, direction, kernel, tile):
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(*shape, seed=6, p=0.75)
-    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
+    compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel, pn.PN_OPT_TILE: tile}, periodic=True)
 
 
 def test_periodic_config_siblings(pn, oracle):
