@@ -84,6 +84,8 @@ typedef struct {
                               entries (they carry a 32-byte overflow record)                               */
     int labels_reused;     /* 1: S1's labelling and peeling were skipped, the classes of the previous solve
                               still hold (pn_update_conductances / pn_replace_conductances, no bond crossed zero) */
+    int residual_recovered;/* 1: the fused kernel ran as persistent launches that store no fp32 residual (it is recovered
+                              from the last two search directions): 36 instead of 40 bytes per node and iteration */
 } pn_info;
 
 /* options for pn_set_option */
@@ -96,7 +98,9 @@ enum {
                                solve axis (default 1; S8(c) reading 6), 2 = warm start: the pressures
                                this handle's previous solve left (S8(f) item 4: re-solves after a
                                change of conductances or direction; first solve: same as 1)         */
-    PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32)            */
+    PN_OPT_CHUNK = 3,       /* inner iterations enqueued between host polls (default 32); the persistent
+                               launches (schemes 5, 6, 7, 8 and 3 with PN_OPT_GRAPH = 1) run to the next residual
+                               replacement, or for this many iterations once the caller has set it  */
     PN_OPT_SKIP_LABEL = 4,  /* 1: skip S1 when the caller guarantees all bonds are open (default 0;
                                S1 is always skipped automatically when no in-lattice g == 0 exists) */
     PN_OPT_KERNEL = 5,      /* inner-iteration kernels: 0 = automatic (5 when the lattice fits one SM's shared

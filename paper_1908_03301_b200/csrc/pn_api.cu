@@ -36,6 +36,7 @@ struct pn_ctx {
     int last_dir_user;
     // options
     int max_iters, chunk, x0_linear, skip_label, variant, profile, peel, lateral;
+    int chunk_set;              // PN_OPT_CHUNK was set by the caller: it also bounds the persistent launches
     int base_closed;            // some in-lattice (non-wrap) bond is closed: from S0's validation
     // node classes kept from the last solve (S8(f) item 4): reused while no bond crosses zero and nothing they depend on changes
     int reuse_labels;           // option
@@ -174,7 +175,7 @@ int pn_create(pn_ctx** out, int nx, int ny, int nz, int device, void* cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->ws = (char*)workspace;
     ctx->ws_bytes = workspace_bytes;
-    ctx->max_iters = 200000; ctx->chunk = 32; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1; ctx->compact = 2; ctx->contract = 1;
+    ctx->max_iters = 200000; ctx->chunk = 32; ctx->chunk_set = 0; ctx->x0_linear = 1; ctx->skip_label = 0; ctx->variant = 0; ctx->peel = 2; ctx->use_graph = 1; ctx->xdefer = 1; ctx->reuse_labels = 1; ctx->compact = 2; ctx->contract = 1;
     ctx->delta = 0.3;   // measured: 0.3 needs 11 % fewer iterations than 0.1 on CFG2 2048^2 and the same on CFG3/4/5
     ctx->last_dir_user = -1;
     // per-handle device facts (no process-global state: handles on different devices are independent)
@@ -249,7 +250,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_MAX_ITERS: if (value < 1 || value > 2e9) return PN_ERR_ARG; ctx->max_iters = (int)value; return PN_OK;
         case PN_OPT_DELTA: if (!(value > 0.0 && value < 1.0)) return PN_ERR_ARG; ctx->delta = value; return PN_OK;
         case PN_OPT_X0: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->x0_linear = (int)value; return PN_OK;
-        case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; return PN_OK;
+        case PN_OPT_CHUNK: if (value < 1 || value > 4096) return PN_ERR_ARG; ctx->chunk = (int)value; ctx->chunk_set = 1; return PN_OK;
         case PN_OPT_SKIP_LABEL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->skip_label = (int)value; return PN_OK;
         case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0 && value != 6.0 && value != 8.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
@@ -413,6 +414,13 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     int scheme = pn_resolve_variant(g, P, ctx->variant);
     int fused = scheme == 3 || scheme == 6 || scheme == 8;   // deferred residual update + predicted beta (the state holds the measured r.r)
     int bufmode = (scheme == 3 || scheme == 8) ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
+    // the fused TMA kernel as one persistent launch per residual replacement (internal launch code 10) stores no residual:
+    // three rotating direction slots (bufmode 3); with periodic faces (k_wrap_fix between the iterations) or PN_OPT_GRAPH = 0
+    // it runs one launch per iteration with stored residuals.  3D tiles only: the 2D tile (lattices above 12 M nodes)
+    // measured slower that way (4096^2: 122.7 against 110.2 us per iteration, 6144^2: 264.7 against 228.5) and keeps the
+    // graph replay of single launches
+    const bool persist_tma = scheme == 3 && ctx->use_graph && g.coop && !any_wrap && g.ny > 1;
+    if (persist_tma) bufmode = 3;
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)
@@ -560,7 +568,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         // 0 the two kernels of an iteration launched one by one
         // the fused TMA kernel likewise (internal code 10), unless periodic faces need k_wrap_fix between the iterations
         const int lscheme = (scheme == 7 && ctx->use_graph && g.coop) ? 9
-                            : ((scheme == 3 && ctx->use_graph && g.coop && !any_wrap) ? 10 : scheme);
+                            : ((scheme == 3 && persist_tma) ? 10 : scheme);
         const bool graph = ctx->use_graph && ctx->chunk > 1 && lscheme < 5 && !(ctx->profile && !fused) && ensure_graph(ctx, scheme, cm, clong);
         const int per_iter = (scheme == 3 ? 1 : 2) + (any_wrap ? 1 : 0);   // (scheme 7: two kernels, never with wrap)
         while (true) {
@@ -570,7 +578,10 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
                 if (ctx->profile) CK(cudaEventRecord(ctx->pev[1], s));
                 nl += per_iter * ctx->chunk;
             } else {
-                CK(pn_launch_inner(g, P, ctx->chunk, lscheme, s, &nl, ctx->profile ? ctx->pev : nullptr, &ctx->C));
+                // (a persistent launch runs up to the next trigger, or PN_OPT_CHUNK iterations when the caller has set it)
+                const bool one_launch = lscheme == 5 || lscheme == 6 || lscheme >= 8;
+                CK(pn_launch_inner(g, P, (one_launch && !ctx->chunk_set) ? (1 << 30) : ctx->chunk, lscheme, s, &nl,
+                                   ctx->profile ? ctx->pev : nullptr, &ctx->C));
             }
             rc = read_state(ctx);
             if (rc) return rc;
@@ -646,6 +657,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         info->n_floating = (long long)h->count[3];
         info->n_peeled = n_peeled;
         info->labels_reused = reuse ? 1 : 0;
+        info->residual_recovered = bufmode == 3 ? 1 : 0;
         info->n_unknowns = cm ? cm : n_solved - n_peeled;
         info->n_chain = (long long)h->n_chain;
         info->n_long_rows = clong;

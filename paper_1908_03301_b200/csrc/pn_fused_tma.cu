@@ -22,7 +22,10 @@
 // non-positive prediction raises the reliable-update flag, i.e. an fp64 residual replacement.
 // r, p and q are double-buffered (index = iteration parity): a tile reads its neighbours' old values as halo.
 //
-// HBM bytes per node: reads r, q, p, x_hat, wx, wy, wz (28 B) + writes r, q, p, x_hat (16 B) = 44 B.
+// HBM bytes per node: reads r, q, p, x_hat, wx, wy, wz (28 B) + writes r, q, p, x_hat (16 B) = 44 B; 40 B with x_hat touched every
+// other iteration; 36 B in the persistent form (PERSIST, 3D tiles), which does not store r at all: r_{t-1} = p_{t-1} -
+// beta_{t-1} p_{t-2} is recovered from the last two search directions, kept in three rotating slots (512^3: 0.8627 -> 0.7473 ms
+// per iteration, same iteration count).
 #include <new>
 
 #include "pn_tma.cuh"
@@ -89,6 +92,11 @@ __device__ __forceinline__ void ft_grid_barrier(unsigned int* bar, unsigned int 
 // tw idle.  A tile step costs ~1.4 us whatever its width against 1.9 us of memory time for a full 256 x 8 tile, so a narrow
 // remainder tile is nearly as expensive as a full one: equal tiles (320^3: 259 -> 252 us) and, more so, the 128 x 16 tile for
 // widths that fill 256-wide tiles badly (252 -> 230 us; FCfg3DN below) keep more of every step's lanes busy.
+// r = ca * p1 + cb * p2 (ca in {0, 1}: exact)
+__device__ __forceinline__ float4 rec4(float ca, const float4& p1, float cb, const float4& p2) {
+    return make_float4(fmaf(cb, p2.x, ca * p1.x), fmaf(cb, p2.y, ca * p1.y), fmaf(cb, p2.z, ca * p1.z), fmaf(cb, p2.w, ca * p1.w));
+}
+
 template <class C, bool PERSIST, bool NARROW>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
 k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int ntx, int nty, int nchunks, int lz,
@@ -133,6 +141,15 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     const float al = (float)st->alpha;          // alpha_{t-1} (0 right after a residual replacement)
     const float nal = -al;
     const int par = st->iters & 1;              // buffers holding r_{t-1}, q_{t-1}, p_{t-1}
+    // PERSIST: the residual is NOT stored (36 instead of 40 bytes per node and iteration).  Three direction slots {P.p, P.p2, P.r}
+    // rotate with the iteration count: p_{t-1} in slot s1, p_{t-2} in s2, p_t goes to s0, and the kernel recovers
+    //     r_{t-1} = p_{t-1} - beta_{t-1} p_{t-2}        (p_{t-1} = r_{t-1} + beta_{t-1} p_{t-2} read backwards; ca = 1, cb = -beta_{t-1})
+    // Right after a residual replacement slot s2 holds the explicit residual k_residual64 wrote: ca = 0, cb = 1.  The recovered
+    // residual differs from a stored one by a rounding of the size of ulp(p); iteration counts are unchanged.
+    const int s1 = st->iters % 3, s2 = (st->iters + 2) % 3, s0 = (st->iters + 1) % 3;
+    const float ca = (PERSIST && !st->rexp) ? 1.f : 0.f;
+    const float cb = PERSIST ? (st->rexp ? 1.f : -(float)st->beta_last) : 1.f;
+    const float a2 = (float)st->alpha2;
     // x_hat is touched every OTHER iteration: xmode 0 = skip (alpha_{t-1} p_{t-1} stays owed), 2 = apply this
     // iteration's update and the owed one, whose direction is recovered as p_{t-2} = (p_{t-1} - r_{t-1}) / beta_{t-1}
     // from values this kernel loads anyway; 1 = plain update (skipping disabled, or beta too small to divide by).
@@ -140,7 +157,7 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     const float c2 = xmode == 2 ? (float)(st->alpha2 / st->beta_prev) : 0.f;
     float* __restrict__ r_out = par ? P.r : P.r2;
     float* __restrict__ q_out = par ? P.q : P.q2;
-    float* __restrict__ p_out = par ? P.p : P.p2;
+    float* __restrict__ p_out = PERSIST ? (s0 == 0 ? P.p : (s0 == 1 ? P.p2 : P.r)) : (par ? P.p : P.p2);
     double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
 
     if (tid >= C::NCONS) {
@@ -169,11 +186,15 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
 #pragma unroll
                     for (int v = 0; v < 3; ++v) {
                         float* sv = sg + v * C::VEC;
+                        // stage regions R_, Q_, P_: r / q / p of the last iteration, or (PERSIST) p_{t-2} / q / p_{t-1} by slot
+                        const int sl = v == 0 ? s2 : s1;
+                        const CUtensorMap* mm = (PERSIST && v != 1) ? (sl == 2 ? &maps.v_main[0][0] : &maps.v_main[2][sl]) : &maps.v_main[v][par];
+                        const CUtensorMap* ms = (PERSIST && v != 1) ? (sl == 2 ? &maps.v_slv[0][0] : &maps.v_slv[2][sl]) : &maps.v_slv[v][par];
 #pragma unroll
                         for (int b = 0; b < C::NBX; ++b)
-                            tma_load_3d(sv + b * C::RH * C::BOXW, &maps.v_main[v][par], x0 + b * C::BOXW, yh, zp, full + s);
-                        tma_load_3d(sv + C::V_SL, &maps.v_slv[v][par], x0 - 4, yh, zp, full + s);
-                        tma_load_3d(sv + C::V_SR, &maps.v_slv[v][par], x0 + txw, yh, zp, full + s);
+                            tma_load_3d(sv + b * C::RH * C::BOXW, mm, x0 + b * C::BOXW, yh, zp, full + s);
+                        tma_load_3d(sv + C::V_SL, ms, x0 - 4, yh, zp, full + s);
+                        tma_load_3d(sv + C::V_SR, ms, x0 + txw, yh, zp, full + s);
                     }
                     if (has_w) {
 #pragma unroll
@@ -235,19 +256,21 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 float4 r_nxt;
                 {
                     const float4 po = lds4(sg + C::P_ + own_main);
-                    const float4 ro = lds4(sg + C::R_ + own_main);      // r_{t-1}
+                    const float4 pR = lds4(sg + C::R_ + own_main);      // r_{t-1}; PERSIST: p_{t-2} (or the explicit residual)
+                    const float4 ro = PERSIST ? rec4(ca, po, cb, pR) : pR;
                     r_nxt = fma4(nal, lds4(sg + C::Q_ + own_main), ro);
                     const float4 pn = fma4(beta, po, r_nxt);
                     if (act) *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
                     if (kk + 1 >= k0 && kk + 1 < k1 && inb) {
                         const long long n = (long long)(kk + 1) * g.plane + nrow;
-                        __stcs(reinterpret_cast<float4*>(r_out + n), r_nxt);
+                        if (!PERSIST) __stcs(reinterpret_cast<float4*>(r_out + n), r_nxt);
                         __stcs(reinterpret_cast<float4*>(p_out + n), pn);
                         if (xmode) {
                             float4 xn = fma4(al, po, xh_use);
                             if (xmode == 2)
-                                xn = make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
-                                                 fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
+                                xn = PERSIST ? fma4(a2, pR, xn)      // the owed direction p_{t-2} is in the stage as it is
+                                             : make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
+                                                           fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
                             __stcs(reinterpret_cast<float4*>(P.xh + n), xn);
                         }
                         a_rr += (double)dot4(r_nxt, r_nxt);
@@ -255,14 +278,16 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 }
                 if (has_halo && (!NARROW || hc4 * 4 < tw)) {
                     const int o = (hb * C::RH + hrow) * bw + hc4 * 4;
-                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
-                    *reinterpret_cast<float4*>(rw + hrow * C::W + 4 + hb * C::BOXW + hc4 * 4) = fma4(beta, lds4(sg + C::P_ + o), rn);
+                    const float4 ph = lds4(sg + C::P_ + o), pRh = lds4(sg + C::R_ + o);
+                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), PERSIST ? rec4(ca, ph, cb, pRh) : pRh);
+                    *reinterpret_cast<float4*>(rw + hrow * C::W + 4 + hb * C::BOXW + hc4 * 4) = fma4(beta, ph, rn);
                 }
                 if (tid < 2 * C::RH) {
                     const int side = tid / C::RH, row = tid - side * C::RH;
                     const int o = (side ? C::V_SR : C::V_SL) + row * 4;
-                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), lds4(sg + C::R_ + o));
-                    *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + txw : 0)) = fma4(beta, lds4(sg + C::P_ + o), rn);
+                    const float4 ps = lds4(sg + C::P_ + o), pRs = lds4(sg + C::R_ + o);
+                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), PERSIST ? rec4(ca, ps, cb, pRs) : pRs);
+                    *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + txw : 0)) = fma4(beta, ps, rn);
                 }
                 if (!C::BAR_END) bar_consumers(C::NCONS);
                 // ---- phase C: q_t(kk) = p_t - W p_t from the ring, weights from the stage.  Of plane kk+1, written just above,

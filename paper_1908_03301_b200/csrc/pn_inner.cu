@@ -345,20 +345,20 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
     if ((scheme == 3 || scheme == 10) && !(pn_tma_supported() && pn_fused_plan_build(&fplan, g, P))) return cudaErrorNotSupported;
     if (scheme == 10) {   // the fused TMA kernel as one persistent cooperative launch up to the next trigger (internal code)
         if (ev) cudaEventRecord(ev[0], st);
-        cudaError_t e10 = pn_launch_cg_fused(fplan, g, P, st, 1 << 30);
+        cudaError_t e10 = pn_launch_cg_fused(fplan, g, P, st, iterations);
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         pn_fused_plan_free(fplan);
         *launches += 1;
         return e10;
     }
-    if (scheme == 5 || scheme == 6 || scheme == 8) {   // the whole loop up to the next trigger in ONE launch (pn_onchip.cu, pn_resident.cu, k_cg_persist); `iterations` is not a bound here
+    if (scheme == 5 || scheme == 6 || scheme == 8) {   // the whole loop up to the next trigger (or `iterations`) in ONE launch (pn_onchip.cu, pn_resident.cu, k_cg_persist)
         if (ev) cudaEventRecord(ev[0], st);
         cudaError_t e5;
-        if (scheme == 5) e5 = pn_launch_cg_onchip(g, P, 1 << 30, st);
-        else if (scheme == 6) e5 = pn_launch_cg_resident(g, P, 1 << 30, st);
+        if (scheme == 5) e5 = pn_launch_cg_onchip(g, P, iterations, st);
+        else if (scheme == 6) e5 = pn_launch_cg_resident(g, P, iterations, st);
         else {
             e5 = cudaMemsetAsync(P.gbar, 0, sizeof(unsigned int), st);
-            int G = g.sms < PN_RESIDENT_MAX_CTAS ? g.sms : PN_RESIDENT_MAX_CTAS, mi = 1 << 30;
+            int G = g.sms < PN_RESIDENT_MAX_CTAS ? g.sms : PN_RESIDENT_MAX_CTAS, mi = iterations;
             pn_geom gg = g;
             pn_ptrs PP = P;
             void* args[] = {(void*)&gg, (void*)&PP, (void*)&mi};
@@ -373,7 +373,7 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
         if (!compact) return cudaErrorInvalidValue;
         if (scheme == 7) return pn_launch_compact_inner(g, P, *compact, iterations, st, launches, ev);
         if (ev) cudaEventRecord(ev[0], st);
-        cudaError_t e9 = pn_launch_compact_persist(g, P, *compact, 1 << 30, st);
+        cudaError_t e9 = pn_launch_compact_persist(g, P, *compact, iterations, st);
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         *launches += 1;
         return e9;

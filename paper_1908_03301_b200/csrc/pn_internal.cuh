@@ -66,8 +66,12 @@ struct pn_state {
     double alpha2;              // alpha of the skipped update (pending on the direction before the current one)
     double beta_prev;           // beta that built the current direction from the skipped one
     double xskip_min;           // skip only while beta >= this (0: never skip)
+    // persistent fused TMA kernel: the residual is not stored, r_{t-1} = p_{t-1} - beta_{t-1} p_{t-2} (pn_fused_tma.cu)
+    double beta_last;           // the beta that built the last direction from the one before (beta_{t-1} for kernel t)
     int xpend;                  // 1: the previous kernel skipped its x_hat update
     int n_xskip;                // iterations of this solve that skipped it (36 instead of 44 B per node)
+    int rexp;                   // 1: first iteration after a residual replacement: r_{t-1} is given explicitly (k_residual64)
+    int pad_;
     double part[4];             // periodic faces: the main kernel's sums, finished by k_wrap_fix (rr, pq, rq, qq | pq)
     double acc[4];              // results of the fp64 reductions (residual norms, b norm, flux)
     unsigned long long count[4];// class counts (solved, inlet-only, outlet-only, floating)
@@ -135,6 +139,8 @@ __device__ __forceinline__ void pn_finish_F(pn_state* st, double rr, double pq, 
     }
     st->alpha = alpha;      // alpha_t: next kernel's residual and solution updates
     st->alpha_x = alpha;    // ... and what k_flush applies to the pending direction p_t
+    st->beta_last = st->beta;   // beta_t built p_t, the direction the next kernel recovers r_t from
+    st->rexp = 0;
     st->beta = beta;
     st->flag = flag;
 }

@@ -30,7 +30,10 @@ __global__ void k_residual64(pn_geom g, pn_ptrs P, int bufmode) {
     __shared__ double sm[32];
     __shared__ double tot[2];
     double a0 = 0.0, a1 = 0.0;
+    // `bufmode` 3: no stored residual (persistent fused TMA kernel): three direction slots {p, p2, r} rotate with the
+    // iteration count; the explicit residual goes where the direction before the last one lay (k_flush is done with it)
     float* __restrict__ rdst = (bufmode == 1 && (P.st->iters & 1)) ? P.r2 : P.r;
+    if (bufmode == 3) { const int sl = (P.st->iters + 2) % 3; rdst = sl == 0 ? P.p : (sl == 1 ? P.p2 : P.r); }
     const bool wrap = g.wrap[0] || g.wrap[1] || g.wrap[2];
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const float s = P.s[n];
@@ -78,12 +81,20 @@ __global__ void k_flush(pn_geom g, pn_ptrs P, int bufmode) {
     const float* __restrict__ p = odd ? P.p2 : P.p;   // the direction of the last iteration
     const float* __restrict__ r = odd ? P.r2 : P.r;   // single-kernel schemes: the residual it was built from
     const bool pend = P.st->xpend != 0;
-    const double c2 = pend ? P.st->alpha2 / P.st->beta_prev : 0.0;
+    double c2 = pend ? P.st->alpha2 / P.st->beta_prev : 0.0;
+    double c1 = 1.0;                                        // dx = x_hat + ax p + c2 (c1 p - r)
+    if (bufmode == 3) {   // direction slots {p, p2, r}: p_T in slot T % 3, p_{T-1} -- what a skipped update is owed on -- in (T + 2) % 3
+        const int s1 = P.st->iters % 3, s2 = (P.st->iters + 2) % 3;
+        p = s1 == 0 ? P.p : (s1 == 1 ? P.p2 : P.r);
+        r = s2 == 0 ? P.p : (s2 == 1 ? P.p2 : P.r);
+        c2 = pend ? -P.st->alpha2 : 0.0;
+        c1 = 0.0;
+    }
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < g.npad; n += (long long)gridDim.x * blockDim.x) {
         const float s = P.s[n];
         if (s != 0.f) {
             double dx = (double)P.xh[n] + ax * (double)p[n];
-            if (pend) dx += c2 * ((double)p[n] - (double)r[n]);
+            if (pend) dx += c2 * (c1 * (double)p[n] - (double)r[n]);
             P.x64[n] += (double)s * dx;
         }
         P.xh[n] = 0.f;
@@ -96,6 +107,8 @@ __global__ void k_set_state(pn_state* st, double rr, double beta, double rr_max,
     st->beta_prev = 0.0;
     st->xskip_min = xskip_min;
     st->xpend = 0;
+    st->beta_last = 0.0;
+    st->rexp = 1;               // the residual k_residual64 has just written is explicit (not recoverable from directions)
     st->rr = rr;
     st->rr_old = rr;
     st->beta = beta;

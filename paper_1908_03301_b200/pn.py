@@ -46,7 +46,8 @@ class PnInfo(ctypes.Structure):
                 ("t_stencil_ms", ctypes.c_double), ("t_update_ms", ctypes.c_double),
                 ("n_timed_iters", ctypes.c_int), ("n_xskip", ctypes.c_int),
                 ("n_peeled", ctypes.c_longlong), ("n_unknowns", ctypes.c_longlong),
-                ("n_chain", ctypes.c_longlong), ("n_long_rows", ctypes.c_longlong), ("labels_reused", ctypes.c_int)]
+                ("n_chain", ctypes.c_longlong), ("n_long_rows", ctypes.c_longlong), ("labels_reused", ctypes.c_int),
+                ("residual_recovered", ctypes.c_int)]
 
 
 @dataclass
@@ -72,6 +73,7 @@ class SolveInfo:
     n_unknowns: int = 0
     n_chain: int = 0
     n_long_rows: int = 0
+    residual_recovered: int = 0
 
 
 class PnError(RuntimeError):
@@ -247,7 +249,7 @@ class Network:
         return SolveInfo(rc, info.outer_cycles, info.inner_iters, info.rel_residual, info.b_norm, info.n_solved,
                          info.n_inlet_only, info.n_outlet_only, info.n_floating, info.t_label_ms, info.t_solve_ms,
                          info.t_stencil_ms, info.t_update_ms, info.n_timed_iters, info.kernel_scheme, info.n_peeled, info.n_xskip,
-                         info.labels_reused, info.n_unknowns, info.n_chain, info.n_long_rows)
+                         info.labels_reused, info.n_unknowns, info.n_chain, info.n_long_rows, info.residual_recovered)
 
     def pressures(self, out=None):
         """fp64 pressures on all nodes as a CUDA tensor of shape (nz, ny, nx)."""

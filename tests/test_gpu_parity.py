@@ -572,11 +572,17 @@ def test_persistent_launch_of_the_tma_kernel(pn, oracle):
     cent (the dot products are grouped per CTA instead of per block), far fewer launches, and bit-reproducible."""
     from paper_1908_03301_b200 import inputs
     for net, d in ((inputs.cfg4_fbm_cut_3d(64, 64, 64), 0), (inputs.iid_diluted(300, 20, 70, seed=5, p=0.75), 2),
-                   (inputs.iid_diluted(2100, 40, 1, seed=9, p=1.0), 1)):
+                   (inputs.iid_diluted(130, 40, 21, seed=9, p=1.0), 1)):
         on, *_ = compare(pn, oracle, net, d, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0})
         off, *_ = compare(pn, oracle, net, d, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0, pn.PN_OPT_GRAPH: 0})
         assert on.kernel_scheme == off.kernel_scheme == 3
+        assert on.residual_recovered == 1 and off.residual_recovered == 0   # persistent launches store no fp32 residual
         assert abs(on.inner_iters - off.inner_iters) <= 0.05 * off.inner_iters + 5
+        for chunk in (1, 2, 3, 7):    # launch boundaries at every phase of the three rotating direction slots
+            cut, *_ = compare(pn, oracle, net, d, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0, pn.PN_OPT_CHUNK: chunk})
+            assert cut.residual_recovered == 1 and abs(cut.inner_iters - on.inner_iters) <= 0.05 * on.inner_iters + 5
+        nodefer, *_ = compare(pn, oracle, net, d, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0, pn.PN_OPT_XDEFER: 0})
+        assert nodefer.residual_recovered == 1 and nodefer.n_xskip == 0
         a = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0})
         b = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0})
         c = gpu_solve(pn, net, d, 1e-10, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_COMPACT: 0, pn.PN_OPT_GRAPH: 0})
@@ -584,6 +590,10 @@ def test_persistent_launch_of_the_tma_kernel(pn, oracle):
         assert a[4] < c[4] / 5                            # launches
     info, *_ = gpu_solve(pn, inputs.cfg2_fbm_2d(300, 200), 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40, pn.PN_OPT_KERNEL: 3})
     assert info.status == pn.PN_MAX_ITERS and info.inner_iters == 40
+    info, *_ = gpu_solve(pn, inputs.cfg4_fbm_cut_3d(40, 36, 33), 0, 1e-12, opts={pn.PN_OPT_MAX_ITERS: 40, pn.PN_OPT_KERNEL: 3})
+    assert info.status == pn.PN_MAX_ITERS and info.inner_iters == 40 and info.residual_recovered == 1
+    flat, *_ = compare(pn, oracle, inputs.iid_diluted(2100, 40, 1, seed=9, p=1.0), 1, opts={pn.PN_OPT_KERNEL: 3})
+    assert flat.kernel_scheme == 3 and flat.residual_recovered == 0     # the 2D tile keeps one launch per iteration (measured faster)
 
 
 @pytest.mark.parametrize("maker,direction,periodic", [
