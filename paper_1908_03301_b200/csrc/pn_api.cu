@@ -414,13 +414,12 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     int scheme = pn_resolve_variant(g, P, ctx->variant);
     int fused = scheme == 3 || scheme == 6 || scheme == 8;   // deferred residual update + predicted beta (the state holds the measured r.r)
     int bufmode = (scheme == 3 || scheme == 8) ? 1 : (scheme == 6 ? 2 : 0);   // where r, q, p live (pn_internal.cuh)
-    // the fused TMA kernel as one persistent launch per residual replacement (internal launch code 10) stores no residual:
-    // three rotating direction slots (bufmode 3); with periodic faces (k_wrap_fix between the iterations) or PN_OPT_GRAPH = 0
-    // it runs one launch per iteration with stored residuals.  3D tiles only: the 2D tile (lattices above 12 M nodes)
-    // measured slower that way (4096^2: 122.7 against 110.2 us per iteration, 6144^2: 264.7 against 228.5) and keeps the
-    // graph replay of single launches
+    // the fused TMA kernel stores no residual: three rotating direction slots (bufmode 3).  It runs as one persistent
+    // launch per residual replacement (internal launch code 10) unless periodic faces need k_wrap_fix between the
+    // iterations or PN_OPT_GRAPH = 0; 3D tiles only: the 2D tile (lattices above 12 M nodes) measured slower that way
+    // and keeps the graph replay of single launches
     const bool persist_tma = scheme == 3 && ctx->use_graph && g.coop && !any_wrap && g.ny > 1;
-    if (persist_tma) bufmode = 3;
+    if (scheme == 3 || scheme == 8) bufmode = 3;   // (k_cg_persist, pn_inner.cu, works the same way)
     int any_closed = ctx->base_closed;
     if (any_wrap) {
         // the forward entries of the last nodes along the wrapping axes are bonds now: copy + validate them (S0's rules)

@@ -79,7 +79,8 @@ struct alignas(64) pn_fmaps {
 // PERSIST: the same kernel as ONE cooperative launch per fp64 residual replacement -- the iteration loop runs inside, the
 // last-block epilogue becomes a grid barrier after which every CTA adds the per-CTA sums in the same fixed order and runs
 // pn_finish_F on its own copy of the state (as k_cg_resident2d / k_cg_persist / k_cpersist do).  Saves the launch gap, the
-// state reads and the reduction tail of every iteration (~17 us of 868 at 512^3); not with periodic faces (k_wrap_fix).
+// state reads and the reduction tail of every iteration (~17 us of 868 at 512^3); not with periodic faces (k_wrap_fix), and
+// not on the 2D tile (measured slower there).
 __device__ __forceinline__ void ft_grid_barrier(unsigned int* bar, unsigned int target) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
     unsigned int v;
@@ -141,23 +142,21 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
     const float al = (float)st->alpha;          // alpha_{t-1} (0 right after a residual replacement)
     const float nal = -al;
     const int par = st->iters & 1;              // buffers holding r_{t-1}, q_{t-1}, p_{t-1}
-    // PERSIST: the residual is NOT stored (36 instead of 40 bytes per node and iteration).  Three direction slots {P.p, P.p2, P.r}
+    // The residual is NOT stored (36 instead of 40 bytes per node and iteration).  Three direction slots {P.p, P.p2, P.r}
     // rotate with the iteration count: p_{t-1} in slot s1, p_{t-2} in s2, p_t goes to s0, and the kernel recovers
     //     r_{t-1} = p_{t-1} - beta_{t-1} p_{t-2}        (p_{t-1} = r_{t-1} + beta_{t-1} p_{t-2} read backwards; ca = 1, cb = -beta_{t-1})
     // Right after a residual replacement slot s2 holds the explicit residual k_residual64 wrote: ca = 0, cb = 1.  The recovered
     // residual differs from a stored one by a rounding of the size of ulp(p); iteration counts are unchanged.
     const int s1 = st->iters % 3, s2 = (st->iters + 2) % 3, s0 = (st->iters + 1) % 3;
-    const float ca = (PERSIST && !st->rexp) ? 1.f : 0.f;
-    const float cb = PERSIST ? (st->rexp ? 1.f : -(float)st->beta_last) : 1.f;
+    const float ca = st->rexp ? 0.f : 1.f;
+    const float cb = st->rexp ? 1.f : -(float)st->beta_last;
     const float a2 = (float)st->alpha2;
     // x_hat is touched every OTHER iteration: xmode 0 = skip (alpha_{t-1} p_{t-1} stays owed), 2 = apply this
-    // iteration's update and the owed one, whose direction is recovered as p_{t-2} = (p_{t-1} - r_{t-1}) / beta_{t-1}
-    // from values this kernel loads anyway; 1 = plain update (skipping disabled, or beta too small to divide by).
+    // iteration's update and the owed one alpha_{t-2} p_{t-2}, whose direction this kernel loads anyway; 1 = plain update
+    // (skipping disabled; a small beta also ends a skip, as in the kernels that recover p_{t-2} by a division).
     const int xmode = st->xpend ? 2 : ((st->xskip_min > 0.0 && st->beta >= st->xskip_min) ? 0 : 1);
-    const float c2 = xmode == 2 ? (float)(st->alpha2 / st->beta_prev) : 0.f;
-    float* __restrict__ r_out = par ? P.r : P.r2;
     float* __restrict__ q_out = par ? P.q : P.q2;
-    float* __restrict__ p_out = PERSIST ? (s0 == 0 ? P.p : (s0 == 1 ? P.p2 : P.r)) : (par ? P.p : P.p2);
+    float* __restrict__ p_out = s0 == 0 ? P.p : (s0 == 1 ? P.p2 : P.r);
     double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
 
     if (tid >= C::NCONS) {
@@ -186,10 +185,10 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
 #pragma unroll
                     for (int v = 0; v < 3; ++v) {
                         float* sv = sg + v * C::VEC;
-                        // stage regions R_, Q_, P_: r / q / p of the last iteration, or (PERSIST) p_{t-2} / q / p_{t-1} by slot
+                        // stage regions R_, Q_, P_: p_{t-2} (or the explicit residual), q_{t-1}, p_{t-1}; directions by slot, q by parity
                         const int sl = v == 0 ? s2 : s1;
-                        const CUtensorMap* mm = (PERSIST && v != 1) ? (sl == 2 ? &maps.v_main[0][0] : &maps.v_main[2][sl]) : &maps.v_main[v][par];
-                        const CUtensorMap* ms = (PERSIST && v != 1) ? (sl == 2 ? &maps.v_slv[0][0] : &maps.v_slv[2][sl]) : &maps.v_slv[v][par];
+                        const CUtensorMap* mm = v != 1 ? (sl == 2 ? &maps.v_main[0][0] : &maps.v_main[2][sl]) : &maps.v_main[1][par];
+                        const CUtensorMap* ms = v != 1 ? (sl == 2 ? &maps.v_slv[0][0] : &maps.v_slv[2][sl]) : &maps.v_slv[1][par];
 #pragma unroll
                         for (int b = 0; b < C::NBX; ++b)
                             tma_load_3d(sv + b * C::RH * C::BOXW, mm, x0 + b * C::BOXW, yh, zp, full + s);
@@ -256,21 +255,17 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 float4 r_nxt;
                 {
                     const float4 po = lds4(sg + C::P_ + own_main);
-                    const float4 pR = lds4(sg + C::R_ + own_main);      // r_{t-1}; PERSIST: p_{t-2} (or the explicit residual)
-                    const float4 ro = PERSIST ? rec4(ca, po, cb, pR) : pR;
+                    const float4 pR = lds4(sg + C::R_ + own_main);      // p_{t-2} (or the explicit residual)
+                    const float4 ro = rec4(ca, po, cb, pR);              // r_{t-1}
                     r_nxt = fma4(nal, lds4(sg + C::Q_ + own_main), ro);
                     const float4 pn = fma4(beta, po, r_nxt);
                     if (act) *reinterpret_cast<float4*>(rw + rrow * C::W + rcol) = pn;
                     if (kk + 1 >= k0 && kk + 1 < k1 && inb) {
                         const long long n = (long long)(kk + 1) * g.plane + nrow;
-                        if (!PERSIST) __stcs(reinterpret_cast<float4*>(r_out + n), r_nxt);
                         __stcs(reinterpret_cast<float4*>(p_out + n), pn);
                         if (xmode) {
                             float4 xn = fma4(al, po, xh_use);
-                            if (xmode == 2)
-                                xn = PERSIST ? fma4(a2, pR, xn)      // the owed direction p_{t-2} is in the stage as it is
-                                             : make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
-                                                           fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
+                            if (xmode == 2) xn = fma4(a2, pR, xn);      // the owed direction p_{t-2} is in the stage as it is
                             __stcs(reinterpret_cast<float4*>(P.xh + n), xn);
                         }
                         a_rr += (double)dot4(r_nxt, r_nxt);
@@ -279,14 +274,14 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 if (has_halo && (!NARROW || hc4 * 4 < tw)) {
                     const int o = (hb * C::RH + hrow) * bw + hc4 * 4;
                     const float4 ph = lds4(sg + C::P_ + o), pRh = lds4(sg + C::R_ + o);
-                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), PERSIST ? rec4(ca, ph, cb, pRh) : pRh);
+                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), rec4(ca, ph, cb, pRh));
                     *reinterpret_cast<float4*>(rw + hrow * C::W + 4 + hb * C::BOXW + hc4 * 4) = fma4(beta, ph, rn);
                 }
                 if (tid < 2 * C::RH) {
                     const int side = tid / C::RH, row = tid - side * C::RH;
                     const int o = (side ? C::V_SR : C::V_SL) + row * 4;
                     const float4 ps = lds4(sg + C::P_ + o), pRs = lds4(sg + C::R_ + o);
-                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), PERSIST ? rec4(ca, ps, cb, pRs) : pRs);
+                    const float4 rn = fma4(nal, lds4(sg + C::Q_ + o), rec4(ca, ps, cb, pRs));
                     *reinterpret_cast<float4*>(rw + row * C::W + (side ? 4 + txw : 0)) = fma4(beta, ps, rn);
                 }
                 if (!C::BAR_END) bar_consumers(C::NCONS);

@@ -143,7 +143,10 @@ __global__ void __launch_bounds__(TPB) k_update(int nvec, pn_ptrs P) {
 // (k_cg_resident2d and k_cpersist work the same way).  r, q, p are double-buffered by iteration parity as in k_cg_fused_tma.
 // A two-phase form (update, barrier, stencil, barrier; single buffers) was measured first: 7.8 / 16.7 / 34.0 us at 64^3 /
 // 128^3 / 2048^2 against 6.5 / 16.1 / 28.5 us for this one.
-constexpr int ST = 1024;
+// Threads per CTA (template parameter ST): 1024 (64 registers: a few spills since the residual is recovered from two
+// directions) streams best on the larger lattices, 768 (80 registers) is faster where latency counts -- measured per iteration,
+// 1024 / 768: 64^3 5.7 / 5.4 us, 128^3 15.2 / 14.2, 160^3 31.9 / 34.9, 2048^2 26.7 / 28.7, 3072^2 56.5 / 60.8; periodic 128^3
+// 21.6 / 17.1.  Chosen by the launcher: 768 with periodic faces and up to 3 M padded nodes.
 
 __device__ __forceinline__ void sp_grid_barrier(unsigned int* bar, unsigned int target) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
@@ -152,20 +155,29 @@ __device__ __forceinline__ void sp_grid_barrier(unsigned int* bar, unsigned int 
     __threadfence();   // acquire; also drops the SM's L1 lines, so that the plain loads that follow see the other CTAs' stores
 }
 
-// p_t at a node from the previous iteration's r, q, p there: the deferred residual update, recomputed wherever needed
-__device__ __forceinline__ float4 pnew4(const float* __restrict__ r, const float* __restrict__ q, const float* __restrict__ p,
-                                        long long n, float nal, float beta) {
-    return fma4(beta, ld4(p + n), fma4(nal, ld4(q + n), ld4(r + n)));
+// No residual is stored (as in k_cg_fused_tma, pn_fused_tma.cu): the directions live in three rotating slots {P.p, P.p2, P.r},
+// p_{t-1} in `p`, p_{t-2} in `p2`, and r_{t-1} = ca p_{t-1} + cb p_{t-2} with (ca, cb) = (1, -beta_{t-1}), or (0, 1) right after a
+// residual replacement, when the slot of p_{t-2} holds the explicit residual k_residual64 wrote.
+struct sp_rec { float ca, cb, nal, beta; };
+__device__ __forceinline__ float4 rec4(const sp_rec& c, const float4& p1, const float4& p2) {
+    return make_float4(fmaf(c.cb, p2.x, c.ca * p1.x), fmaf(c.cb, p2.y, c.ca * p1.y), fmaf(c.cb, p2.z, c.ca * p1.z), fmaf(c.cb, p2.w, c.ca * p1.w));
 }
-__device__ __forceinline__ float pnew1(const float* __restrict__ r, const float* __restrict__ q, const float* __restrict__ p,
-                                       long long n, float nal, float beta) {
-    return fmaf(beta, p[n], fmaf(nal, q[n], r[n]));
+// p_t at a node from the previous iteration's p_{t-2}, q, p_{t-1} there: the deferred residual update, recomputed wherever needed
+__device__ __forceinline__ float4 pnew4(const float* __restrict__ p2, const float* __restrict__ q, const float* __restrict__ p,
+                                        long long n, const sp_rec& c) {
+    const float4 p1 = ld4(p + n);
+    return fma4(c.beta, p1, fma4(c.nal, ld4(q + n), rec4(c, p1, ld4(p2 + n))));
+}
+__device__ __forceinline__ float pnew1(const float* __restrict__ p2, const float* __restrict__ q, const float* __restrict__ p,
+                                       long long n, const sp_rec& c) {
+    const float p1 = p[n];
+    return fmaf(c.beta, p1, fmaf(c.nal, q[n], fmaf(c.cb, p2[n], c.ca * p1)));
 }
 
 // WRAP: periodic lateral faces.  A node on a wrapping face has one more bond, to the node on the
 // opposite face, weight in the face array ww (pn_setup.cu k_wrap_weights; zero on pad columns); its p_t is recomputed from
 // r, q, p there like any other neighbour's: no second kernel (k_wrap_fix, pn_wrap.cu) and no second barrier.
-template <bool WRAP>
+template <bool WRAP, int ST>
 __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int max_launch_iters) {
     pn_state* st = P.st;
     if (st->flag != PN_FLAG_RUN) return;   // same value in every CTA: nobody enters the barrier alone
@@ -189,25 +201,25 @@ __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int 
 
     for (int li = 0; li < max_launch_iters; ++li) {
         const int pin = li & 1;
-        const int par = ls.iters & 1;                               // buffers holding r_{t-1}, q_{t-1}, p_{t-1}
-        const float* __restrict__ r = par ? P.r2 : P.r;
+        const int par = ls.iters & 1;                               // buffer holding q_{t-1}
+        const int s1 = ls.iters % 3, s2 = (ls.iters + 2) % 3, s0 = (ls.iters + 1) % 3;   // slots of p_{t-1}, p_{t-2}, p_t
+        const float* __restrict__ r = s2 == 0 ? P.p : (s2 == 1 ? P.p2 : P.r);   // p_{t-2} (or the explicit residual): r_{t-1} is recovered
         const float* __restrict__ q = par ? P.q2 : P.q;
-        const float* __restrict__ p = par ? P.p2 : P.p;
-        float* __restrict__ r_out = par ? P.r : P.r2;
+        const float* __restrict__ p = s1 == 0 ? P.p : (s1 == 1 ? P.p2 : P.r);
         float* __restrict__ q_out = par ? P.q : P.q2;
-        float* __restrict__ p_out = par ? P.p : P.p2;
-        const float al = (float)ls.alpha, nal = -al, beta = (float)ls.beta;
+        float* __restrict__ p_out = s0 == 0 ? P.p : (s0 == 1 ? P.p2 : P.r);
+        const float al = (float)ls.alpha, nal = -al, beta = (float)ls.beta, a2 = (float)ls.alpha2;
+        const sp_rec rc{ls.rexp ? 0.f : 1.f, ls.rexp ? 1.f : -(float)ls.beta_last, nal, beta};
         // x_hat every other iteration, exactly as in k_cg_fused_tma
         const int xmode = ls.xpend ? 2 : ((ls.xskip_min > 0.0 && ls.beta >= ls.xskip_min) ? 0 : 1);
-        const float c2 = xmode == 2 ? (float)(ls.alpha2 / ls.beta_prev) : 0.f;
         double a_rr = 0.0, a_pq = 0.0, a_rq = 0.0, a_qq = 0.0;
         for (long long v = v0 + tid; v < v1; v += ST) {
             const long long n = 4 * v;
-            const float4 ro = ld4(r + n), po = ld4(p + n);
-            const float4 rn = fma4(nal, ld4(q + n), ro);
+            const float4 p2o = ld4(r + n), po = ld4(p + n);
+            const float4 rn = fma4(nal, ld4(q + n), rec4(rc, po, p2o));
             const float4 pn = fma4(beta, po, rn);
-            const float pl = pnew1(r, q, p, n - 1, nal, beta), pr = pnew1(r, q, p, n + 4, nal, beta);
-            const float4 pzm = pnew4(r, q, p, n - plane, nal, beta), pzp = pnew4(r, q, p, n + plane, nal, beta);
+            const float pl = pnew1(r, q, p, n - 1, rc), pr = pnew1(r, q, p, n + 4, rc);
+            const float4 pzm = pnew4(r, q, p, n - plane, rc), pzp = pnew4(r, q, p, n + plane, rc);
             const float4 gx = ld4(wx + n), gz = ld4(wz + n), gzm = ld4(wz + n - plane);
             const float gxl = wx[n - 1];
             float4 s;
@@ -216,7 +228,7 @@ __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int 
             s.z = gx.y * pn.y + gx.z * pn.w + gzm.z * pzm.z + gz.z * pzp.z;
             s.w = gx.z * pn.z + gx.w * pr + gzm.w * pzm.w + gz.w * pzp.w;
             if (has_y) {
-                const float4 pym = pnew4(r, q, p, n - px, nal, beta), pyp = pnew4(r, q, p, n + px, nal, beta);
+                const float4 pym = pnew4(r, q, p, n - px, rc), pyp = pnew4(r, q, p, n + px, rc);
                 const float4 gy = ld4(wy + n), gym = ld4(wy + n - px);
                 s.x += gym.x * pym.x + gy.x * pyp.x;
                 s.y += gym.y * pym.y + gy.y * pyp.y;
@@ -229,34 +241,31 @@ __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int 
                 if (g.wrap[0]) {
                     const int last = g.nx - 1, e = last - i0;
                     const float w0 = P.ww[0][j + (long long)g.ny * k];
-                    if (i0 == 0) s.x += w0 * pnew1(r, q, p, n + last, nal, beta);
+                    if (i0 == 0) s.x += w0 * pnew1(r, q, p, n + last, rc);
                     if (e >= 0 && e < 4) {
-                        const float t = w0 * pnew1(r, q, p, n + e - last, nal, beta);
+                        const float t = w0 * pnew1(r, q, p, n + e - last, rc);
                         if (e == 0) s.x += t; else if (e == 1) s.y += t; else if (e == 2) s.z += t; else s.w += t;
                     }
                 }
                 if (g.wrap[1] && (j == 0 || j == g.ny - 1)) {
                     const long long sp = (long long)(g.ny - 1) * px;
                     const float4 w1 = ld4(P.ww[1] + i0 + (long long)px * k);
-                    const float4 pp = pnew4(r, q, p, j == 0 ? n + sp : n - sp, nal, beta);
+                    const float4 pp = pnew4(r, q, p, j == 0 ? n + sp : n - sp, rc);
                     s.x += w1.x * pp.x; s.y += w1.y * pp.y; s.z += w1.z * pp.z; s.w += w1.w * pp.w;
                 }
                 if (g.wrap[2] && (k == 0 || k == g.nz - 1)) {
                     const long long sp = (long long)(g.nz - 1) * plane;
                     const float4 w2 = ld4(P.ww[2] + i0 + (long long)px * j);
-                    const float4 pp = pnew4(r, q, p, k == 0 ? n + sp : n - sp, nal, beta);
+                    const float4 pp = pnew4(r, q, p, k == 0 ? n + sp : n - sp, rc);
                     s.x += w2.x * pp.x; s.y += w2.y * pp.y; s.z += w2.z * pp.z; s.w += w2.w * pp.w;
                 }
             }
             const float4 qv = make_float4(pn.x - s.x, pn.y - s.y, pn.z - s.z, pn.w - s.w);
-            st4(r_out + n, rn);
             st4(p_out + n, pn);
             st4(q_out + n, qv);
             if (xmode) {
                 float4 xn = fma4(al, po, ld4(P.xh + n));
-                if (xmode == 2)
-                    xn = make_float4(fmaf(c2, po.x - ro.x, xn.x), fmaf(c2, po.y - ro.y, xn.y),
-                                     fmaf(c2, po.z - ro.z, xn.z), fmaf(c2, po.w - ro.w, xn.w));
+                if (xmode == 2) xn = fma4(a2, p2o, xn);       // the owed alpha_{t-2} p_{t-2}
                 st4(P.xh + n, xn);
             }
             a_rr += (double)(rn.x * rn.x + rn.y * rn.y + rn.z * rn.z + rn.w * rn.w);
@@ -271,7 +280,7 @@ __global__ void __launch_bounds__(ST, 1) k_cg_persist(pn_geom g, pn_ptrs P, int 
             double* my = P.slots + ((size_t)pin * PN_MAX_BLOCKS + c) * 4;     // [parity][CTA][4]: one 32-byte sector per CTA
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const double v = pn_warp_sum(red[32 * k + lane]);
+                const double v = pn_warp_sum(lane < ST / 32 ? red[32 * k + lane] : 0.0);
                 if (lane == 0) my[k] = v;
             }
             if (lane == 0) { bar_target += G; sp_grid_barrier(bar, bar_target); }
@@ -362,8 +371,10 @@ cudaError_t pn_launch_inner(const pn_geom& g, const pn_ptrs& P, int iterations, 
             pn_geom gg = g;
             pn_ptrs PP = P;
             void* args[] = {(void*)&gg, (void*)&PP, (void*)&mi};
-            const void* fn = (g.wrap[0] | g.wrap[1] | g.wrap[2]) ? (const void*)k_cg_persist<true> : (const void*)k_cg_persist<false>;
-            if (e5 == cudaSuccess) e5 = cudaLaunchCooperativeKernel(fn, dim3(G), dim3(ST), args, 0, st);
+            const bool wrap8 = (g.wrap[0] | g.wrap[1] | g.wrap[2]) != 0, few = wrap8 || g.npad <= 3000000;
+            const void* fn = wrap8 ? (const void*)k_cg_persist<true, 768>
+                                   : (few ? (const void*)k_cg_persist<false, 768> : (const void*)k_cg_persist<false, 1024>);
+            if (e5 == cudaSuccess) e5 = cudaLaunchCooperativeKernel(fn, dim3(G), dim3(few ? 768 : 1024), args, 0, st);
         }
         if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
         *launches += 1;

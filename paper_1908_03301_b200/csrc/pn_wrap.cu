@@ -29,7 +29,15 @@ __global__ void __launch_bounds__(TPB) k_wrap_fix(pn_geom g, pn_ptrs P, int fuse
     const int par = st->iters & 1;                       // same parity the main kernel of this iteration used
     const float* __restrict__ p = par ? P.p : P.p2;      // p_t, written by the main kernel
     float* __restrict__ q = fused ? (par ? P.q : P.q2) : P.q;
-    const float* __restrict__ r = par ? P.r : P.r2;      // r_t (single-kernel scheme only)
+    // single-kernel scheme: no stored residual; directions in three rotating slots {p, p2, r} (pn_fused_tma.cu):
+    // p_t in slot (iters + 1) % 3, p_{t-1} in slot iters % 3, and r_t = p_t - beta_t p_{t-1}
+    const float* __restrict__ pm = nullptr;
+    const float beta_t = (float)st->beta;
+    if (fused) {
+        const int s0 = (st->iters + 1) % 3, s1 = st->iters % 3;
+        p = s0 == 0 ? P.p : (s0 == 1 ? P.p2 : P.r);
+        pm = s1 == 0 ? P.p : (s1 == 1 ? P.p2 : P.r);
+    }
     const int dims[3] = {g.nx, g.ny, g.nz};
     double d_pq = 0.0, d_qq = 0.0, d_rq = 0.0;
     for (int b = 0; b < 3; ++b) {
@@ -62,7 +70,7 @@ __global__ void __launch_bounds__(TPB) k_wrap_fix(pn_geom g, pn_ptrs P, int fuse
             d_pq += (double)(p[n] * dq);
             if (fused) {
                 d_qq += (double)(2.f * qo * dq + dq * dq);
-                d_rq += (double)(r[n] * dq);
+                d_rq += (double)(fmaf(-beta_t, pm[n], p[n]) * dq);
             }
         }
     }
