@@ -135,7 +135,9 @@ enum {
     PN_OPT_GRAPH = 9,       /* 1 (default): a chunk of inner iterations is replayed from a CUDA graph (captured
                                once per geometry / direction / scheme); with the compacted unknowns (scheme 7): ONE
                                persistent cooperative launch runs all iterations up to the next residual
-                               replacement.  0: every kernel launched directly, one by one                  */
+                               replacement.  0: every kernel launched directly, one by one.  2: as 1, and the 2D tile of
+                               scheme 3 runs as a persistent launch too (it measured slower than graph replay and is
+                               not chosen automatically; kept for measurements)                              */
     PN_OPT_REUSE_LABELS = 11, /* 1 (default): a solve that follows pn_update_conductances / pn_replace_conductances (or simply
                                repeats the previous one) keeps the node classes, pins and peeled set of the previous solve
                                when no bond went from closed to open or back and direction, PN_OPT_LATERAL, PN_OPT_PEEL

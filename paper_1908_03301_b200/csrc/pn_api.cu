@@ -255,7 +255,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_KERNEL: if (value != 0.0 && value != 1.0 && value != 3.0 && value != 5.0 && value != 6.0 && value != 8.0) return PN_ERR_ARG; ctx->variant = (int)value; return PN_OK;
         case PN_OPT_PROFILE: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->profile = (int)value; return PN_OK;
         case PN_OPT_LATERAL: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->lateral = (int)value; return PN_OK;
-        case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
+        case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
         case PN_OPT_CONTRACT: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->contract = (int)value; return PN_OK;
         case PN_OPT_TILE: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->g.tile = (int)value; return PN_OK;
@@ -418,7 +418,7 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
     // launch per residual replacement (internal launch code 10) unless periodic faces need k_wrap_fix between the
     // iterations or PN_OPT_GRAPH = 0; 3D tiles only: the 2D tile (lattices above 12 M nodes) measured slower that way
     // and keeps the graph replay of single launches
-    const bool persist_tma = scheme == 3 && ctx->use_graph && g.coop && !any_wrap && g.ny > 1;
+    const bool persist_tma = scheme == 3 && ctx->use_graph && g.coop && !any_wrap && (g.ny > 1 || ctx->use_graph == 2);
     if (scheme == 3 || scheme == 8) bufmode = 3;   // (k_cg_persist, pn_inner.cu, works the same way)
     int any_closed = ctx->base_closed;
     if (any_wrap) {
@@ -548,6 +548,9 @@ static int solve_impl(pn_ctx* ctx, int direction, double tol, pn_info* info, int
         status = PN_NO_SPANNING_CLUSTER;
         rn = 0.0;
     } else if (rn > tol * nb) {
+        // (a smaller threshold for the compacted scheme, whose replacements cost 12 iterations' worth each, was tried: 0.1 saves
+        // 6 % on CFG3 256^3 -- 17 -> 10 replacements, same 2135 iterations -- but costs 16 % more iterations on a harder
+        // near-threshold case of the test suite, 18780 against 16233: 0.3 stays the default everywhere)
         const double delta2 = ctx->delta * ctx->delta;
         const double xskip_min = (fused && scheme != 7 && ctx->xdefer) ? 0.1 : 0.0;   // x_hat updated every other iteration (pn_fused_tma.cu)
         auto target_for = [&](double rn_true, double rr_true) {
