@@ -87,7 +87,7 @@ inline bool make_map(CUtensorMap* m, const pn_geom& g, const float* base_with_ha
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// z-chunk length of the 2.5D march: balance the persistent grid against the `extra_bytes_per_chunk_node` every
+// z-chunk length of the 2.5D march (2D tile): balance the persistent grid against the `extra_bytes_per_chunk_node` every
 // chunk pays for its two extra leading planes (per node of a plane, against `bytes_per_node` of useful traffic)
 inline int choose_lz(int nz, int tiles, int nblocks, double bytes_per_node, double extra_bytes_per_chunk_node, int max_lz = 64) {
     int best = 1;
@@ -101,6 +101,38 @@ inline int choose_lz(int nz, int tiles, int nblocks, double bytes_per_node, doub
         const double eff = balance * halo;
         if (eff > best_eff + 1e-9) { best_eff = eff; best = lz; }
     }
+    return best;
+}
+
+// z-chunks of the 2.5D march (3D tiles).  The nz planes of every tile are cut into `nchunks` EQUAL parts (chunk j = planes
+// [j nz / nchunks, (j+1) nz / nchunks)); item = (chunk, tile), CTA c of the persistent grid takes items c, c + G, ...
+// Every item pays two extra leading planes (its prologue).  Chosen: the count that minimises the plane steps of the
+// busiest CTA, computed exactly; ties go to fewer chunks (less prologue traffic).  (Round 1 fixed a chunk LENGTH and
+// left a ragged last chunk: 494 steps per CTA instead of 462 at 512^3, 40 instead of 34 at 192^3.)
+inline int choose_chunks(int nz, int tiles, int nblocks) {
+    thread_local int last_key[3] = {0, 0, 0}, last_val = 0;   // launchers ask again for every launch
+    if (last_key[0] == nz && last_key[1] == tiles && last_key[2] == nblocks) return last_val;
+    int best = 1;
+    long long best_cost = -1;
+    int max_chunks = nz / 4 > 1 ? nz / 4 : 1;
+    long long cap = (8ll * nblocks + tiles - 1) / tiles;   // up to ~8 items per CTA, or 8 chunks per tile: beyond, only more prologues
+    if (cap < 8) cap = 8;
+    if (max_chunks > cap) max_chunks = (int)cap;
+    for (int nch = 1; nch <= max_chunks; ++nch) {
+        const long long items = (long long)nch * tiles;
+        long long cost = 0;
+        const long long ncta = items < nblocks ? items : nblocks;
+        for (long long c = 0; c < ncta; ++c) {
+            long long tot = 0;
+            for (long long it = c; it < items; it += nblocks) {
+                const long long j = it / tiles;
+                tot += ((j + 1) * nz / nch - j * nz / nch) + 2;
+            }
+            if (tot > cost) cost = tot;
+        }
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = nch; }
+    }
+    last_key[0] = nz; last_key[1] = tiles; last_key[2] = nblocks; last_val = best;
     return best;
 }
 
