@@ -167,11 +167,11 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                 const int chunk = item / tiles, t = item - chunk * tiles;
                 const int tyi = t / ntx, txi = t - tyi * ntx;
                 const int x0 = txi * txw, y0 = tyi * C::TY;
-                // z-chunks: nchunks equal parts (3D tiles); fixed length lz, ragged last chunk (2D tile).  A compile-time choice:
+                // z-chunks: nchunks equal parts (3D tiles; 32-bit: chunk < 1200, nz < 2^21); fixed length lz, ragged last chunk (2D tile).  A compile-time choice:
                 // the 2D instantiation is sensitive to its code generation (a run-time choice here cost it 27 %, 98 -> 125 us
                 // per iteration at 4096^2, with 85 instead of 76 registers and the same chunks)
-                const int k0 = C::HAS_Y ? (int)((long long)chunk * g.nz / nchunks) : chunk * lz;
-                const int k1 = C::HAS_Y ? (int)((long long)(chunk + 1) * g.nz / nchunks) : min(k0 + lz, g.nz);
+                const int k0 = C::HAS_Y ? (int)((unsigned)chunk * (unsigned)g.nz / (unsigned)nchunks) : chunk * lz;
+                const int k1 = C::HAS_Y ? (int)((unsigned)(chunk + 1) * (unsigned)g.nz / (unsigned)nchunks) : min(k0 + lz, g.nz);
                 const int yh = y0 - (C::HAS_Y ? 1 : 0);
                 const unsigned b_rqp = NARROW ? 3u * (unsigned)(C::RH * bw + 2 * C::RH * 4) * 4u : C::B_RQP;
                 const unsigned b_w = NARROW ? (unsigned)(C::TY * bw + C::TY * 4 + (C::HAS_Y ? C::RWY * bw : 0)) * 4u : C::B_W;
@@ -236,8 +236,8 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
             const int chunk = item / tiles, t = item - chunk * tiles;
             const int tyi = t / ntx, txi = t - tyi * ntx;
             const int x0 = txi * txw, y0 = tyi * C::TY;
-            const int k0 = C::HAS_Y ? (int)((long long)chunk * g.nz / nchunks) : chunk * lz;
-            const int k1 = C::HAS_Y ? (int)((long long)(chunk + 1) * g.nz / nchunks) : min(k0 + lz, g.nz);
+            const int k0 = C::HAS_Y ? (int)((unsigned)chunk * (unsigned)g.nz / (unsigned)nchunks) : chunk * lz;
+            const int k1 = C::HAS_Y ? (int)((unsigned)(chunk + 1) * (unsigned)g.nz / (unsigned)nchunks) : min(k0 + lz, g.nz);
             const int x = x0 + b * C::BOXW + c4 * 4, y = y0 + ty;
             const bool inb = act && (x < g.px) && (y < g.ny);
             const long long nrow = (long long)y * g.px + x;
