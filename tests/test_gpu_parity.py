@@ -934,3 +934,45 @@ def test_chain_elimination_hand_built(pn, oracle):
     for peel in (0, 1):
         info, *_ = compare(pn, oracle, net, 0, tol=1e-13, opts={pn.PN_OPT_COMPACT: 1, pn.PN_OPT_KERNEL: 3, pn.PN_OPT_PEEL: peel})
         assert info.kernel_scheme == 7 and info.n_chain > 40
+
+
+# ---- seeded random configurations: shapes, dilution, direction, faces, kernels, tiles and launch cuts drawn together ----
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_random_configurations(pn, oracle, seed):
+    """40 cases per seed through the same element-by-element comparison as everything above: 2D and 3D shapes up to
+    ~530 wide (several TMA tiles, both 3D tile shapes, equal narrow tiles), p from 1 down to 0.4, all solve axes,
+    periodic faces, every kernel scheme, persistent launches cut after 1 .. 5 iterations, with and without the deferred
+    solution update, peeling, graph replay and the zero start."""
+    from paper_1908_03301_b200 import inputs
+    rng = np.random.default_rng(seed)
+    done = 0
+    while done < 40:
+        if rng.random() < 0.7:
+            shape = [int(rng.integers(3, 90)), int(rng.integers(1, 40)), int(rng.integers(1, 40))]
+            if rng.random() < 0.25:
+                shape[0] = int(rng.integers(250, 530))
+            if rng.random() < 0.3:
+                rng.shuffle(shape)
+        else:
+            shape = [int(rng.integers(3, 400)), int(rng.integers(3, 120)), 1]
+            if rng.random() < 0.2:
+                shape[0] = int(rng.integers(2040, 2200))
+        nx, ny, nz = shape
+        axes = [d for d in range(3 if nz > 1 else 2) if shape[d] >= 3]
+        if not axes:
+            continue
+        direction = int(rng.choice(axes))
+        p = float(rng.choice([1.0, 0.85, 0.6, 0.4]))
+        periodic = bool(rng.random() < 0.35)
+        kernel = int(rng.choice([0, 1, 3, 3, 8, 8]))
+        opts = {pn.PN_OPT_KERNEL: kernel}
+        if kernel == 3:
+            opts[pn.PN_OPT_TILE] = int(rng.choice([0, 1, 2]))
+        if rng.random() < 0.3:
+            opts[pn.PN_OPT_CHUNK] = int(rng.choice([1, 2, 3, 5, 64]))
+        for key, values in ((pn.PN_OPT_GRAPH, [0]), (pn.PN_OPT_XDEFER, [0]), (pn.PN_OPT_PEEL, [0, 1]), (pn.PN_OPT_X0, [0])):
+            if rng.random() < 0.2:
+                opts[key] = int(rng.choice(values))
+        net = inputs.iid_diluted(nx, ny, nz, seed=int(rng.integers(1 << 30)), p=p)
+        compare(pn, oracle, net, direction, tol=1e-13, opts=opts, periodic=periodic)
+        done += 1
