@@ -157,9 +157,10 @@ enum {
                                reason for the slow convergence there.  0: never.  Pressures of all
                                nodes stay those of the full system                                            */
     PN_OPT_TILE = 14,       /* tile of the fused TMA kernel (scheme 3) on 3D lattices: 1 = 256 x 8 nodes, 2 = 128 x 16,
-                               0 (default) = automatic: 128 x 16 where it fills its lanes at least 8 % better (widths such as
-                               320 or 384 that leave a 256-wide tile mostly empty); with either, a width that does not fill
-                               its last tile is cut into equal tiles                                           */
+                               3 = 64 x 32, 0 (default) = automatic: a narrower tile where it fills its lanes at least 8 %
+                               better than the next wider one (widths such as 192, 320 or 384 that leave a 256-wide tile
+                               mostly empty); with any of them a width that does not fill its last tile is cut into equal
+                               tiles                                                                           */
     PN_OPT_XDEFER = 10      /* 1 (default): the single-kernel scheme applies the fp32 solution update every OTHER
                                iteration, two search directions at once (the earlier one recovered from p and r):
                                40 instead of 44 bytes per node-iteration on average; 0: every iteration    */

@@ -258,7 +258,7 @@ int pn_set_option(pn_ctx* ctx, int key, double value) {
         case PN_OPT_GRAPH: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->use_graph = (int)value; return PN_OK;
         case PN_OPT_XDEFER: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->xdefer = (int)value; return PN_OK;
         case PN_OPT_CONTRACT: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->contract = (int)value; return PN_OK;
-        case PN_OPT_TILE: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->g.tile = (int)value; return PN_OK;
+        case PN_OPT_TILE: if (value != 0.0 && value != 1.0 && value != 2.0 && value != 3.0) return PN_ERR_ARG; ctx->g.tile = (int)value; return PN_OK;
         case PN_OPT_COMPACT: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->compact = (int)value; return PN_OK;
         case PN_OPT_REUSE_LABELS: if (value != 0.0 && value != 1.0) return PN_ERR_ARG; ctx->reuse_labels = (int)value; return PN_OK;
         case PN_OPT_PEEL: if (value != 0.0 && value != 1.0 && value != 2.0) return PN_ERR_ARG; ctx->peel = (int)value; return PN_OK;

@@ -44,8 +44,8 @@ struct FCfg {
     // tile uses LDS / STS (see the kernel's first lines)
     static constexpr bool BAR_END = true;
     static constexpr int BOXW = BOXW_;                     // nodes per box row (256 = the TMA box limit per dimension)
-    static constexpr int LPR = BOXW / 4;                   // consumer lanes per box row (whole warps)
-    static_assert(BOXW % 128 == 0 && BOXW <= 256, "box rows of whole warps");
+    static constexpr int LPR = BOXW / 4;                   // consumer lanes per box row (64, 32 or 16: whole warps, or two rows per warp)
+    static_assert(BOXW % 64 == 0 && BOXW <= 256, "box rows of whole or half warps");
     static constexpr int TXW = BOXW * NBX;                 // tile width in nodes
     static constexpr int RH = TY + (HAS_Y ? 2 : 0);        // rows of r, q, p and p_new including the y halo
     static constexpr int RWY = TY + (HAS_Y ? 1 : 0);       // rows of the wy box (backward row included)
@@ -300,11 +300,11 @@ k_cg_fused_tma(const __grid_constant__ pn_fmaps maps, pn_geom g, pn_ptrs P, int 
                     const float4 pzp = lds4(rw + rrow * C::W + rcol);
                     float pl = __shfl_up_sync(0xffffffffu, pc.w, 1);
                     float pr = __shfl_down_sync(0xffffffffu, pc.x, 1);
-                    if (lane == 0) pl = r0[-1];
-                    if (lane == 31) pr = r0[4];
+                    if (lane == 0 || (C::LPR < 32 && c4 == 0)) pl = r0[-1];          // (c4 tests: a warp holds two rows when LPR == 16)
+                    if (lane == 31 || (C::LPR < 32 && c4 == C::LPR - 1)) pr = r0[4];
                     const float4 gx = lds4(sg + C::WX + own_ty);
                     float gxl = __shfl_up_sync(0xffffffffu, gx.w, 1);
-                    if (lane == 0) {
+                    if (lane == 0 || (C::LPR < 32 && c4 == 0)) {
                         if (c4 != 0) gxl = sg[C::WX + own_ty - 1];
                         else if (b != 0) gxl = sg[C::WX + ((b - 1) * C::TY + ty) * C::BOXW + C::BOXW - 1];   // (b != 0: never NARROW)
                         else gxl = sg[C::WX_SL + ty * 4 + 3];
@@ -452,6 +452,7 @@ cudaError_t launch_cfg(const pn_geom& g, const pn_ptrs& P, const pn_fmaps& M, in
 
 typedef FCfg<1, 8, true, 3> FCfg3D;    // 256 x 8 tile, y halo, 3 stages
 typedef FCfg<1, 16, true, 3, 128> FCfg3DN;   // 128 x 16 tile for widths that fill 256-wide tiles badly (e.g. 320, 384)
+typedef FCfg<1, 32, true, 3, 64> FCfg3DS;    // 64 x 32 tile for widths that fill 128-wide tiles badly too (e.g. 192, 320)
 typedef FCfg<8, 1, false, 4> FCfg2D;   // 2048 x 1 tile (lattices held as nx x 1 x ny), 4 stages
 
 // fraction of the consumer lanes of a tiling that hold lattice nodes
@@ -475,6 +476,10 @@ cudaError_t pn_fused_init_device() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DN, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DN::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DS, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DS::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DS::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DS::SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg3DS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg3DS::SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cg_fused_tma<FCfg2D, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FCfg2D::SMEM_BYTES);
     return e;
@@ -482,19 +487,29 @@ cudaError_t pn_fused_init_device() {
 
 struct pn_fused_plan {
     pn_fmaps maps;
-    int kind;      // 0: 2D tile, 1: 256 x 8, 2: 128 x 16
+    int kind;      // 0: 2D tile, 1: 256 x 8, 2: 128 x 16, 3: 64 x 32
 };
 
 bool pn_fused_plan_build(pn_fused_plan** out, const pn_geom& g, const pn_ptrs& P) {
     if (!get_encoder()) return false;
     pn_fused_plan* pl = new (std::nothrow) pn_fused_plan;
     if (!pl) return false;
-    // 3D: the 128 x 16 tile where it fills its lanes at least 8 % better than the 256 x 8 one, which is the faster of the two on
-    // widths both fill (512^3: 0.861 against 0.884 ms per iteration; 256^3: 113.8 against 115.2 us).  Measured with the tile
-    // forced either way (profiles/r02_small_lattices.md): 320^3 252 -> 230 us, 384^3 392 -> 371 us, 260^3 161 -> 143 us
-    pl->kind = g.ny == 1 ? 0 : (g.tile ? g.tile : (lane_efficiency<FCfg3DN>(g) > 1.08 * lane_efficiency<FCfg3D>(g) ? 2 : 1));
+    // 3D: a narrower, taller tile where it fills its lanes at least 8 % better than the next wider one; of two that fill
+    // equally the wider is the faster (512^3: 0.861 against 0.884 ms per iteration for 256 x 8 / 128 x 16; 256^3: 113.8 against
+    // 115.2 us).  Measured with the tile forced (profiles/r02_small_lattices.md): 320^3 252 -> 230 us, 384^3 392 -> 371 us,
+    // 260^3 161 -> 143 us with 128 x 16
+    if (g.ny == 1) pl->kind = 0;
+    else if (g.tile) pl->kind = g.tile;
+    else {
+        const double e1 = lane_efficiency<FCfg3D>(g), e2 = lane_efficiency<FCfg3DN>(g), e3 = lane_efficiency<FCfg3DS>(g);
+        pl->kind = 1;
+        double best = e1;
+        if (e2 > 1.08 * best) { pl->kind = 2; best = e2; }
+        if (e3 > 1.08 * best) { pl->kind = 3; best = e3; }
+    }
     const bool ok = pl->kind == 0 ? build_maps<FCfg2D>(&pl->maps, g, P)
-                                  : (pl->kind == 1 ? build_maps<FCfg3D>(&pl->maps, g, P) : build_maps<FCfg3DN>(&pl->maps, g, P));
+                    : (pl->kind == 1 ? build_maps<FCfg3D>(&pl->maps, g, P)
+                                     : (pl->kind == 2 ? build_maps<FCfg3DN>(&pl->maps, g, P) : build_maps<FCfg3DS>(&pl->maps, g, P)));
     if (!ok) { delete pl; return false; }
     *out = pl;
     return true;
@@ -506,5 +521,6 @@ void pn_fused_plan_free(pn_fused_plan* pl) { delete pl; }
 // next trigger (no periodic faces)
 cudaError_t pn_launch_cg_fused(const pn_fused_plan* pl, const pn_geom& g, const pn_ptrs& P, cudaStream_t st, int max_launch_iters) {
     if (pl->kind == 0) return launch_cfg<FCfg2D>(g, P, pl->maps, max_launch_iters, st);
-    return pl->kind == 1 ? launch_cfg<FCfg3D>(g, P, pl->maps, max_launch_iters, st) : launch_cfg<FCfg3DN>(g, P, pl->maps, max_launch_iters, st);
+    if (pl->kind == 1) return launch_cfg<FCfg3D>(g, P, pl->maps, max_launch_iters, st);
+    return pl->kind == 2 ? launch_cfg<FCfg3DN>(g, P, pl->maps, max_launch_iters, st) : launch_cfg<FCfg3DS>(g, P, pl->maps, max_launch_iters, st);
 }

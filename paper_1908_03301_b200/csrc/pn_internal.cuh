@@ -34,7 +34,7 @@ struct pn_geom {
     int wrap[3];                // INTERNAL axis wraps around (periodic lateral faces); never `dir`, never a length-1 axis
     int sms;                    // SM count of the handle's device (sizes the persistent grids); set by pn_create
     int coop;                   // the device launches cooperative kernels (pn_resident.cu)
-    int tile;                   // PN_OPT_TILE: 3D tile of the fused TMA kernel (0 automatic, 1: 256 x 8, 2: 128 x 16)
+    int tile;                   // PN_OPT_TILE: 3D tile of the fused TMA kernel (0 automatic, 1: 256 x 8, 2: 128 x 16, 3: 64 x 32)
 };
 
 // ---- periodic lateral faces: the wrap bonds live in small FACE arrays, not in the lattice-shaped ones ----

@@ -135,14 +135,15 @@ def test_ragged_2d(pn, oracle, shape, direction, p, kernel):
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel})
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3])
 @pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0), ((256, 33, 9), 0),
-                                             ((130, 40, 21), 1)])
+                                             ((130, 40, 21), 1), ((192, 70, 33), 2), ((66, 5, 40), 0)])
 def test_tma_kernel_multi_tile(pn, oracle, shape, direction, tile):
     """Lattices wider than one TMA box and taller than one tile: x and y halos between tiles, several z chunks, ragged
-    tails in all three directions.  Both 3D tiles (PN_OPT_TILE: 256 x 8 and 128 x 16 nodes; 0 = automatic); widths that do
-    not fill their last tile are cut into EQUAL narrower tiles (260 -> 2 x 132 or 3 x 88; 300 -> 2 x 152 or 3 x 100;
-    520 -> 3 x 176 or 5 x 104; 130 -> 1 x 132 or 2 x 68), 256 is the one exact fit."""
+    tails in all three directions.  All three 3D tiles (PN_OPT_TILE: 256 x 8, 128 x 16 and 64 x 32 nodes -- the last with two
+    lattice rows per warp; 0 = automatic); widths that do not fill their last tile are cut into EQUAL narrower tiles
+    (260 -> 2 x 132, 3 x 88 or 5 x 52; 300 -> 2 x 152, 3 x 100 or 5 x 60; 520 -> 3 x 176, 5 x 104 or 9 x 60; 130 -> 1 x 132,
+    2 x 68 or 3 x 44; 66 -> 1 x 68 or 2 x 36), 256 and 192 = 3 x 64 are exact fits."""
     from paper_1908_03301_b200 import inputs
     net = inputs.iid_diluted(*shape, seed=5, p=0.75)
     info, *_ = compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: 3, pn.PN_OPT_TILE: tile})
@@ -467,7 +468,7 @@ def test_periodic_ragged_2d(pn, oracle, shape, direction, kernel):
     compare(pn, oracle, net, direction, opts={pn.PN_OPT_KERNEL: kernel}, periodic=True)
 
 
-@pytest.mark.parametrize("kernel,tile", [(3, 1), (3, 2), (8, 0)])
+@pytest.mark.parametrize("kernel,tile", [(3, 1), (3, 2), (3, 3), (8, 0)])
 @pytest.mark.parametrize("shape,direction", [((300, 20, 70), 2), ((520, 9, 12), 1), ((260, 17, 40), 0)])
 def test_periodic_multi_tile(pn, oracle, shape, direction, kernel, tile):
     from paper_1908_03301_b200 import inputs
@@ -967,7 +968,7 @@ def test_random_configurations(pn, oracle, seed):
         kernel = int(rng.choice([0, 1, 3, 3, 8, 8]))
         opts = {pn.PN_OPT_KERNEL: kernel}
         if kernel == 3:
-            opts[pn.PN_OPT_TILE] = int(rng.choice([0, 1, 2]))
+            opts[pn.PN_OPT_TILE] = int(rng.choice([0, 1, 2, 3]))
         if rng.random() < 0.3:
             opts[pn.PN_OPT_CHUNK] = int(rng.choice([1, 2, 3, 5, 64]))
         for key, values in ((pn.PN_OPT_GRAPH, [0]), (pn.PN_OPT_XDEFER, [0]), (pn.PN_OPT_PEEL, [0, 1]), (pn.PN_OPT_X0, [0])):
