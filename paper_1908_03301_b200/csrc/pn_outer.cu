@@ -26,7 +26,10 @@ int grid_for(long long work_items, int sms) {
 // (b - A x)_i = sum_j g_ij (x_j - x_i) over all six neighbours.  acc[0] = ||r||^2, acc[1] = ||r_hat||^2
 // (of the rounded fp32 values, i.e. exactly what the inner recurrence starts from).
 // `bufmode` 1: the single-kernel iteration double-buffers r; the next kernel reads buffer (iters & 1).
-__global__ void k_residual64(pn_geom g, pn_ptrs P, int bufmode) {
+// 8 blocks per SM (32 registers, ~60 bytes of spills): the kernel is bound by the latency of its scattered fp64 loads, not by
+// registers -- ncu at 512^3 (profiles/r02_ncu.md): 72 registers gave 34 % of the warps and 2192 us (24 % of the DRAM rate),
+// 64 registers 1150 us, 32 registers 1020 us; 256^3: 299 -> 138 us
+__global__ void __launch_bounds__(TPB, 8) k_residual64(pn_geom g, pn_ptrs P, int bufmode) {
     __shared__ double sm[32];
     __shared__ double tot[2];
     double a0 = 0.0, a1 = 0.0;
