@@ -155,7 +155,10 @@ enum {
                                P:53) -- and take the resistance-weighted interpolation of the end pressures afterwards.
                                Near the threshold these "links" are 69 % of the unknowns left after peeling and the
                                reason for the slow convergence there.  0: never.  Pressures of all
-                               nodes stay those of the full system                                            */
+                               nodes stay those of the full system.  Safety net: if the iteration on the reduced
+                               system breaks down or stagnates before its budget is spent, pn_solve repeats the
+                               solve once on the lattice kernels, without elimination and compaction (pn_info then
+                               reports n_chain = 0, that kernel_scheme and the iterations of both attempts)    */
     PN_OPT_TILE = 14,       /* tile of the fused TMA kernel (scheme 3) on 3D lattices: 1 = 256 x 8 nodes, 2 = 128 x 16,
                                3 = 64 x 32, 0 (default) = automatic: a narrower tile where it fills its lanes at least 8 %
                                better than the next wider one (widths such as 192, 320 or 384 that leave a 256-wide tile

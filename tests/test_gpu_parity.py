@@ -977,3 +977,35 @@ def test_random_configurations(pn, oracle, seed):
         net = inputs.iid_diluted(nx, ny, nz, seed=int(rng.integers(1 << 30)), p=p)
         compare(pn, oracle, net, direction, tol=1e-13, opts=opts, periodic=periodic)
         done += 1
+
+
+def test_link_elimination_safety_net(pn, oracle):
+    """tests/golden/chain_case_53x22x7.npz: a near-threshold network (p = 0.35, every open bond drifted by 1 %) found by a
+    random stress run of the update path: the SECOND solve on a handle whose first solve had eliminated the links broke
+    down (-6) or stagnated, whatever the second network's path.  Cause: the compacted scheme and the chain records borrow
+    lattice arrays and left garbage in their halo planes, which the iteration kernels read as zeros; pn_solve now zeroes
+    the halos at every solve (and repeats a solve that fails with the links eliminated on the plain lattice kernels).
+    The network alone, and sequences on one handle through set / replace, must meet the full parity bar."""
+    import os
+    from types import SimpleNamespace
+    d = np.load(os.path.join(os.path.dirname(__file__), "golden", "chain_case_53x22x7.npz"))
+    net = SimpleNamespace(nx=53, ny=22, nz=7, gx=d["gx"], gy=d["gy"], gz=d["gz"], name="chain_case_53x22x7", n_nodes=53 * 22 * 7)
+    direction = int(d["direction"])
+    info, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_PEEL: 1})
+    assert info.status == pn.PN_OK
+    plain, *_ = compare(pn, oracle, net, direction, tol=1e-13, opts={pn.PN_OPT_PEEL: 1, pn.PN_OPT_CONTRACT: 0})
+    assert plain.status == pn.PN_OK and plain.n_chain == 0
+    # on one handle: a good network, the bad one through pn_replace_conductances (label reuse, warm start), a good one again
+    from paper_1908_03301_b200 import inputs
+    h = pn.Network(53, 22, 7)
+    h.set_option(pn.PN_OPT_PEEL, 1)
+    good = inputs.iid_diluted(53, 22, 7, seed=4, p=0.35)
+    for arrays in ((good.gx, good.gy, good.gz), (d["gx"], d["gy"], d["gz"]), (good.gx, good.gy, good.gz)):
+        h.set_conductances(*arrays) if arrays[0] is good.gx else h.replace_conductances(*arrays)
+        got = h.solve(direction, 1e-13, accept=(pn.PN_OK, pn.PN_NO_SPANNING_CLUSTER))
+        if got.status != pn.PN_OK:
+            continue
+        ref = oracle.solve(53, 22, 7, arrays[0], arrays[1], arrays[2], direction, 1e-13)
+        assert np.max(np.abs(h.pressures().cpu().numpy() - ref.P)) <= 1e-8
+        assert abs(h.flux()[2] - ref.g_eff) <= 1e-9 * abs(ref.g_eff)
+    h.close()
